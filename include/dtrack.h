@@ -1,0 +1,196 @@
+/*
+ * dtrack.h -- C ABI of the B200-native non-linear digital-tracking hot path.
+ *
+ * What the library computes (BASELINE.json north_star; the
+ * paper gives the skeleton only: Algorithm 1 PAPER.md:149-176 `SearchImages` ->
+ * `FilterGPUIntersections` -> `FindLocalSignal` -> combine -> `FindSignificantResults`, and
+ * PAPER.md:141-143, 202 "orbital parameters -> sky position at the image time -> location within
+ * the pixel grid -> keep intersections inside image bounds -> pull pixels -> jointly combine"):
+ *
+ *   for every candidate orbit o = (a, e, i, Omega, omega, M0 at epoch t0) and every exposure j
+ *     1. n = sqrt(GM/a^3), M = M0 + n (t_j - t0), solve E - e sin E = M            (fp64)
+ *     2. r = a(cos E - e) P + a sqrt(1-e^2) sin E Q          (heliocentric ecliptic)
+ *     3. ONE light-time iteration: tau = |r(t_j) - R_j| / c, r' = r(t_j - tau); observer stays at t_j
+ *     4. d = r' - R_j, rotate ecliptic -> equatorial by the obliquity
+ *     5. gnomonic (TAN) projection about the exposure's tangent point, +x east, +y north,
+ *        x = (W-1)/2 + xi/s, y = (H-1)/2 + eta/s, nearest pixel ix = floor(x + 1/2)
+ *     6. cull unless D > 0 and 0 <= x + 1/2 < W and 0 <= y + 1/2 < H
+ *     7. gather f = flux_j[iy][ix] and v = var_j[iy][ix] (or the exposure's scalar variance);
+ *        skip the hit unless f, v finite and v > 0
+ *     8. per orbit, ascending exposure: S += f/v, Wt += 1/v, hits += 1;  SNR = S / sqrt(Wt), 0 if
+ *        hits == 0
+ *   dt_topk: the k largest SNR (ties: lower orbit index first) among orbits with hits >= min_hits.
+ *
+ * Every step runs in hand-written sm_100a CUDA kernels; there is NO CPU fallback: every compute
+ * call returns DT_ERR_CUDA when no CUDA device is usable.  Units: AU, days, radians.
+ *
+ * Conventions
+ *   - every call returns a status: 0 = DT_OK, negative = error; nothing throws or aborts across
+ *     the ABI.  dt_last_error(ctx) returns a context-owned, NUL-terminated string that stays valid
+ *     until the next call on that context (a static string when ctx == NULL).
+ *   - pointers are tagged by a `mem_kind` argument: DT_MEM_HOST (pageable host), DT_MEM_PINNED
+ *     (page-locked host) or DT_MEM_DEVICE (device memory of the context's device).
+ *   - ownership: dt_create copies all metadata; the caller owns every input and output buffer.
+ *     The one exception is documented at dt_load_image_batch (streaming mode retains the pointer).
+ *   - one context per host thread; no global state; a context is bound to one CUDA device/stream.
+ */
+#ifndef DTRACK_H
+#define DTRACK_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dt_context dt_context; /* opaque */
+
+enum {
+    DT_OK = 0,
+    DT_ERR_INVALID_ARG = -1,
+    DT_ERR_OOM = -2,
+    DT_ERR_CUDA = -3,
+    DT_ERR_NOT_LOADED = -4,
+    DT_ERR_STATE = -5
+};
+enum { DT_MEM_HOST = 0, DT_MEM_PINNED = 1, DT_MEM_DEVICE = 2 };
+
+/* dt_survey.flags */
+enum {
+    DT_FLAG_FORCE_STREAM = 1,   /* never keep images resident: always stream batches from host     */
+    DT_FLAG_KEPLER_COLD = 2,    /* solve every pair from a cold start with libdevice sincos        */
+                                /* (reference mode of kernel 1; default is the warm-started solve) */
+    DT_FLAG_NO_PRECULL = 4      /* do the light-time refinement + projection for every pair, even  */
+                                /* when a conservative cone test already proves a miss             */
+};
+
+/*
+ * Exposure metadata (Algorithm 1 `image_list` + the per-image header record of PAPER.md:202,
+ * "a few hundred bytes of data for each image").  All arrays are HOST pointers, copied by
+ * dt_create.  All exposures share width x height (true of all five BASELINE.json configs).
+ */
+typedef struct {
+    uint32_t struct_size;      /* sizeof(dt_survey): ABI versioning, must match                   */
+    int32_t n_exposures;       /* N >= 1                                                          */
+    int32_t width, height;     /* pixels; 1 <= W, H and W*H < 2^31                                */
+    const double *t;           /* [N] exposure mid-times, days                                    */
+    const double *obs_ecl;     /* [N][3] heliocentric ECLIPTIC observer position at t[j], AU      */
+    const double *ra0;         /* [N] tangent point right ascension, rad                          */
+    const double *dec0;        /* [N] tangent point declination, rad                              */
+    double pixel_scale;        /* rad per pixel, > 0                                              */
+    double gm;                 /* AU^3/day^2; NaN => 2.959122082855911e-4 (Gaussian k^2)          */
+    double c;                  /* AU/day; NaN => 173.14463267424033; +inf => no light-time        */
+    double obliquity;          /* rad; NaN => 0.40909262775014904 (23.439281 deg)                 */
+    int32_t variance_mode;     /* 0: per-exposure scalar var_scalar[N]; 1: fp32 plane per exposure */
+    const double *var_scalar;  /* [N], mode 0 (ignored in mode 1)                                 */
+    int32_t device;            /* CUDA device ordinal                                             */
+    void *stream;              /* cudaStream_t supplied by the caller (e.g. torch's current       */
+                               /* stream); NULL = the legacy default stream                       */
+    int64_t hbm_budget_bytes;  /* device bytes the image store may use; 0 => 75% of free memory   */
+    uint32_t flags;            /* DT_FLAG_*                                                       */
+} dt_survey;
+
+/* Counters of the most recent dt_stack call (dt_get_stats). */
+typedef struct {
+    uint32_t struct_size;
+    int64_t n_orbits, n_exposures;
+    int64_t pairs;             /* n_orbits * n_exposures                                          */
+    int64_t hits;              /* footprint hits written by the cull+compaction stage             */
+    int64_t invalid_orbits;    /* orbits rejected (a <= 0, e outside [0,1), non-finite)           */
+    int64_t refined_pairs;     /* pairs that went through light-time refinement + projection      */
+    int64_t cold_solves;       /* Kepler solves started cold (libdevice sincos Newton)            */
+    int64_t h2d_image_bytes;   /* image bytes streamed host -> device inside the call             */
+    int32_t streamed;          /* 1 when the image store did not fit and batches were streamed    */
+    int32_t n_image_batches;   /* exposure ranges processed                                       */
+    float ms_total;            /* whole call, CUDA events on the context stream                   */
+    float ms_propagate;        /* kernel 1+2 (propagate, project, cull, compact), summed          */
+    float ms_gather;           /* kernel 3 (gather + stack), summed                               */
+    float ms_finalize;         /* SNR finalisation                                                */
+    int32_t launches;          /* kernels launched by the call                                    */
+    int32_t propagate_launches, gather_launches;
+} dt_stats;
+
+/*
+ * dt_create: build a context for a survey.  Computes and uploads the per-exposure constant records
+ * (observer rotated to the equatorial frame, tangent-plane basis scaled by 1/pixel_scale, variance).
+ * Errors: DT_ERR_INVALID_ARG (NULL / size mismatch / non-positive sizes / non-finite metadata),
+ * DT_ERR_CUDA (no device, or a CUDA call failed), DT_ERR_OOM.
+ */
+int dt_create(const dt_survey *survey, dt_context **out);
+int dt_destroy(dt_context *ctx);
+
+/*
+ * dt_load_image_batch: register the difference images of exposures [first, first+count)
+ * (Algorithm 1 `LoadImages`).  flux (and var in variance_mode 1, else NULL) point to
+ * count contiguous planes [count][H][W] of fp32 in the memory named by mem_kind.
+ *   - if the whole survey fits hbm_budget_bytes (and DT_FLAG_FORCE_STREAM is not set) the planes
+ *     are COPIED into the context's image store in HBM and the caller may free them on return;
+ *   - otherwise (streaming mode; north_star subsystem 4) the library RETAINS the pointers: they
+ *     must be DT_MEM_PINNED (else DT_ERR_INVALID_ARG) and stay valid until dt_destroy or until the
+ *     same exposure range is loaded again; dt_stack then streams them in double-buffered batches.
+ * Ranges may be loaded in any order and re-loaded; overlapping a previously loaded range replaces it.
+ */
+int dt_load_image_batch(dt_context *ctx, int32_t first_exposure, int32_t count, const float *flux,
+                        const float *var, int32_t mem_kind);
+
+/*
+ * dt_stack: the hot path (steps 1-8 above) for n orbits against all exposures.
+ *   elements  [n][6] = a (AU), e, i, Omega, omega, M0 (rad), fp64, in memory `mem_kind`
+ *   t0        epoch of M0, days (one per call)
+ *   snr_out   [n] fp64, hits_out [n] int32, in memory `mem_kind` (either may be NULL)
+ * Invalid orbits do not fail the call: they get hits = -1, snr = NaN.  Results are complete when
+ * the call returns (the call synchronises the context stream).  The per-orbit results also stay
+ * on the device for dt_topk.  Errors: DT_ERR_NOT_LOADED unless every exposure has images.
+ */
+int dt_stack(dt_context *ctx, const double *elements, int64_t n, double t0, int32_t mem_kind,
+             double *snr_out, int32_t *hits_out);
+
+/*
+ * dt_topk: the k largest SNR of the most recent dt_stack, SNR descending, ties by orbit index
+ * ascending, over orbits with hits >= min_hits and finite SNR (Algorithm 1 `FindSignificantResults`,
+ * PAPER.md:173).  index_out [k] int64, snr_out [k] fp64 are HOST pointers; *n_found = min(k, count).
+ * Errors: DT_ERR_STATE when no dt_stack result exists; DT_ERR_INVALID_ARG for k < 0.
+ */
+int dt_topk(dt_context *ctx, int32_t k, int32_t min_hits, int64_t *index_out, double *snr_out,
+            int32_t *n_found);
+
+/*
+ * dt_project: parity/debug entry (not on the timed path): steps 1-6 for every pair, written densely.
+ *   radec_out [n][N][2] (alpha in [0, 2pi), delta), xy_out [n][N][2] (x, y), pix_out [n][N][2]
+ *   ((-1,-1) when culled).  HOST pointers; any may be NULL.  Uses the same device functions as
+ *   dt_stack's kernel 1 (mode selected by the context flags).
+ */
+int dt_project(dt_context *ctx, const double *elements, int64_t n, double t0, double *radec_out,
+               double *xy_out, int32_t *pix_out);
+
+/*
+ * dt_gather_hits: kernel 3 on a caller-supplied hit list (micro-benchmark / test entry).
+ * The hit list uses the library's internal orbit-major format for ONE exposure range
+ * [first_exposure, first_exposure + 32*n_groups): for group g and orbit o, bit b of
+ * mask[g*n_pad + o] says orbit o hits exposure first_exposure + 32 g + b; the pixel offsets
+ * (iy*W + ix) of warp-tile w = o/32 in group g start at offsets[base[g*(n_pad/32) + w]], orbit-major
+ * then exposure-ascending.  n_pad = n rounded up to 32.  All pointers are DEVICE pointers.
+ * Accumulates into S[n], Wt[n] (fp64) and cnt[n] (int32), which the caller zero-initialises.
+ * Images must be resident (DT_ERR_STATE in streaming mode).
+ */
+int dt_gather_hits(dt_context *ctx, int64_t n, int32_t first_exposure, int32_t n_groups,
+                   const uint32_t *mask, const uint64_t *base, const uint32_t *offsets, double *S,
+                   double *Wt, int32_t *cnt);
+
+int dt_get_stats(const dt_context *ctx, dt_stats *out);
+const char *dt_last_error(const dt_context *ctx);
+
+/* Library build information: "dtrack-b200 <version> sm_100a". */
+const char *dt_version(void);
+
+/*
+ * dt_fp64_peak: measures the device's FP64 FMA issue rate with a register-resident DFMA loop
+ * (the "alu" roofline denominator of kernel 1; MEASURED_PEAKS.json has no FP64 figure).
+ * Writes achieved TFLOP/s (2 flop per DFMA) to *tflops.  device: CUDA ordinal.
+ */
+int dt_fp64_peak(int32_t device, double *tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DTRACK_H */

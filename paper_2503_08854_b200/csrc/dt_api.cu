@@ -1,0 +1,659 @@
+// dt_api.cu -- the C ABI (include/dtrack.h): context, image store and batch scheduler, dt_stack
+// orchestration, dt_project, dt_topk, statistics.  Host code only launches kernels and moves
+// bytes; every step of the hot path runs in the kernels of dt_propagate.cu / dt_gather.cu /
+// dt_topk.cu.  There is no CPU fallback: without a usable CUDA device every call fails.
+#include "../../include/dtrack.h"
+
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "dt_common.cuh"
+
+using namespace dt;
+
+namespace {
+
+constexpr int64_t kMaxUnitOrbits = 1 << 20;   // orbits per work unit (bounds the hit buffer)
+constexpr int32_t kMaxUnitExposures = 512;    // exposures per work unit (16 groups)
+constexpr int kMinCtas = 148 * 4;             // fill the machine before giving up exposure splits
+
+struct Timer {
+    cudaEvent_t a = nullptr, b = nullptr;
+};
+
+}  // namespace
+
+struct dt_context {
+    int device = 0;
+    cudaStream_t stream = nullptr, copy_stream = nullptr;
+    bool own_stream = false;
+    int32_t N = 0, W = 0, H = 0;
+    int64_t plane = 0;
+    int32_t var_mode = 0;
+    uint32_t flags = 0;
+    double pixel_scale = 0, gm = 0, c = 0, inv_c = 0, obliq = 0, cos_eps = 1, sin_eps = 0, tan_fov = 0;
+    std::vector<ExpRec> h_exp;
+    ExpRec *d_exp = nullptr;
+
+    // image store
+    bool streaming = false;
+    int64_t budget = 0;
+    float *d_flux = nullptr, *d_var = nullptr;          // resident: N planes each
+    std::vector<uint8_t> loaded;                        // per exposure
+    std::vector<const float *> h_flux, h_var;           // streaming: retained pinned pointers
+    float *d_buf_flux[2] = {nullptr, nullptr}, *d_buf_var[2] = {nullptr, nullptr};
+    int32_t batch_exp = 0;
+    cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
+    bool ev_free_recorded[2] = {false, false};
+
+    // orbit-side buffers
+    double *d_el = nullptr;
+    int64_t el_cap = 0;
+    double *d_S = nullptr, *d_Wt = nullptr, *d_snr = nullptr;
+    int32_t *d_cnt = nullptr, *d_hits = nullptr;
+    int64_t acc_cap = 0, n_last = -1;
+    uint32_t *d_mask = nullptr;
+    unsigned long long *d_base = nullptr;
+    uint32_t *d_offsets = nullptr;
+    int64_t mask_cap = 0, base_cap = 0, off_cap = 0;
+    unsigned long long *d_counters = nullptr;           // [8]
+    std::vector<cudaEvent_t> ev_pool;                   // timing events
+
+    TopkWorkspace topk;
+    dt_stats stats;
+    std::string err;
+};
+
+namespace {
+
+const char *g_static_err = "dtrack: invalid context";
+
+int fail(dt_context *ctx, int code, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (ctx) ctx->err = buf;
+    return code;
+}
+
+#define CU(ctx, call)                                                                          \
+    do {                                                                                       \
+        cudaError_t e__ = (call);                                                              \
+        if (e__ != cudaSuccess)                                                                \
+            return fail(ctx, e__ == cudaErrorMemoryAllocation ? DT_ERR_OOM : DT_ERR_CUDA,      \
+                        "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e__), __FILE__,     \
+                        __LINE__);                                                             \
+    } while (0)
+
+template <typename T>
+cudaError_t grow(T *&ptr, int64_t &cap, int64_t need)
+{
+    if (ptr && need <= cap) return cudaSuccess;
+    if (ptr) cudaFree(ptr);
+    ptr = nullptr;
+    cap = 0;
+    if (need <= 0) need = 1;
+    cudaError_t e = cudaMalloc((void **)&ptr, (size_t)need * sizeof(T));
+    if (e == cudaSuccess) cap = need;
+    return e;
+}
+
+void free_all(dt_context *c)
+{
+    cudaFree(c->d_exp);
+    cudaFree(c->d_flux);
+    cudaFree(c->d_var);
+    for (int s = 0; s < 2; ++s) {
+        cudaFree(c->d_buf_flux[s]);
+        cudaFree(c->d_buf_var[s]);
+        if (c->ev_ready[s]) cudaEventDestroy(c->ev_ready[s]);
+        if (c->ev_free[s]) cudaEventDestroy(c->ev_free[s]);
+    }
+    cudaFree(c->d_el);
+    cudaFree(c->d_S);
+    cudaFree(c->d_Wt);
+    cudaFree(c->d_snr);
+    cudaFree(c->d_cnt);
+    cudaFree(c->d_hits);
+    cudaFree(c->d_mask);
+    cudaFree(c->d_base);
+    cudaFree(c->d_offsets);
+    cudaFree(c->d_counters);
+    for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    topk_free(c->topk);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
+}
+
+// Per-exposure constant record (hot-path step 2): observer rotated to the equatorial frame,
+// tangent-plane basis (east, north) divided by the pixel scale, tangent unit vector.
+ExpRec make_record(const dt_context *c, double t, const double *obs, double ra0, double dec0, double var)
+{
+    ExpRec r;
+    memset(&r, 0, sizeof r);
+    r.t = t;
+    r.Rx = obs[0];
+    r.Ry = obs[1] * c->cos_eps - obs[2] * c->sin_eps;
+    r.Rz = obs[1] * c->sin_eps + obs[2] * c->cos_eps;
+    const double sa = sin(ra0), ca = cos(ra0), sd = sin(dec0), cd = cos(dec0);
+    const double is = 1.0 / c->pixel_scale;
+    r.ex = -sa * is;
+    r.ey = ca * is;
+    r.ez = 0.0;
+    r.nx = -sd * ca * is;
+    r.ny = -sd * sa * is;
+    r.nz = cd * is;
+    r.tx = cd * ca;
+    r.ty = cd * sa;
+    r.tz = sd;
+    r.var = var;
+    r.inv_var = 1.0 / var;
+    return r;
+}
+
+int mem_kind_ok(int32_t k) { return k == DT_MEM_HOST || k == DT_MEM_PINNED || k == DT_MEM_DEVICE; }
+
+int ensure_store(dt_context *c)
+{
+    if (c->streaming) {
+        if (c->d_buf_flux[0]) return DT_OK;
+        const int64_t per_exp = c->plane * 4 * (c->var_mode == 1 ? 2 : 1);
+        int64_t b = c->budget / (2 * per_exp);
+        if (b < 1) return fail(c, DT_ERR_OOM, "hbm_budget_bytes %lld cannot hold two exposures of %lld bytes",
+                               (long long)c->budget, (long long)per_exp);
+        b = std::min<int64_t>(b, kMaxUnitExposures);
+        b = std::min<int64_t>(b, c->N);
+        if (b >= kGroup) b -= b % kGroup;
+        c->batch_exp = (int32_t)b;
+        for (int s = 0; s < 2; ++s) {
+            CU(c, cudaMalloc((void **)&c->d_buf_flux[s], (size_t)(b * c->plane) * 4));
+            if (c->var_mode == 1) CU(c, cudaMalloc((void **)&c->d_buf_var[s], (size_t)(b * c->plane) * 4));
+            CU(c, cudaEventCreateWithFlags(&c->ev_ready[s], cudaEventDisableTiming));
+            CU(c, cudaEventCreateWithFlags(&c->ev_free[s], cudaEventDisableTiming));
+        }
+        return DT_OK;
+    }
+    if (!c->d_flux) CU(c, cudaMalloc((void **)&c->d_flux, (size_t)(c->N * c->plane) * 4));
+    if (c->var_mode == 1 && !c->d_var) CU(c, cudaMalloc((void **)&c->d_var, (size_t)(c->N * c->plane) * 4));
+    return DT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *dt_version(void) { return "dtrack-b200 0.1 sm_100a"; }
+
+const char *dt_last_error(const dt_context *ctx) { return ctx ? ctx->err.c_str() : g_static_err; }
+
+int dt_create(const dt_survey *s, dt_context **out)
+{
+    if (!out) return DT_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!s || s->struct_size != sizeof(dt_survey)) return DT_ERR_INVALID_ARG;
+    if (s->n_exposures < 1 || s->width < 1 || s->height < 1 ||
+        (int64_t)s->width * s->height >= ((int64_t)1 << 31))
+        return DT_ERR_INVALID_ARG;
+    if (!s->t || !s->obs_ecl || !s->ra0 || !s->dec0) return DT_ERR_INVALID_ARG;
+    if (!(s->pixel_scale > 0.0) || !isfinite(s->pixel_scale)) return DT_ERR_INVALID_ARG;
+    if (s->variance_mode != 0 && s->variance_mode != 1) return DT_ERR_INVALID_ARG;
+    if (s->variance_mode == 0 && !s->var_scalar) return DT_ERR_INVALID_ARG;
+    for (int32_t j = 0; j < s->n_exposures; ++j) {
+        if (!isfinite(s->t[j]) || !isfinite(s->ra0[j]) || !isfinite(s->dec0[j]) ||
+            !isfinite(s->obs_ecl[3 * j]) || !isfinite(s->obs_ecl[3 * j + 1]) ||
+            !isfinite(s->obs_ecl[3 * j + 2]))
+            return DT_ERR_INVALID_ARG;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1 || s->device < 0 || s->device >= ndev) {
+        cudaGetLastError();
+        return DT_ERR_CUDA;   // no CPU fallback
+    }
+    dt_context *c = new (std::nothrow) dt_context();
+    if (!c) return DT_ERR_OOM;
+    memset(&c->stats, 0, sizeof c->stats);
+    c->stats.struct_size = sizeof(dt_stats);
+    c->device = s->device;
+    if (cudaSetDevice(c->device) != cudaSuccess) { delete c; return DT_ERR_CUDA; }
+    c->N = s->n_exposures;
+    c->W = s->width;
+    c->H = s->height;
+    c->plane = (int64_t)s->width * s->height;
+    c->var_mode = s->variance_mode;
+    c->flags = s->flags;
+    c->pixel_scale = s->pixel_scale;
+    c->gm = isnan(s->gm) ? 2.959122082855911025e-4 : s->gm;
+    c->c = isnan(s->c) ? 173.14463267424033 : s->c;
+    c->obliq = isnan(s->obliquity) ? 0.40909262775014904 : s->obliquity;
+    if (!(c->gm > 0.0) || !(c->c > 0.0)) { delete c; return DT_ERR_INVALID_ARG; }
+    c->inv_c = isinf(c->c) ? 0.0 : 1.0 / c->c;
+    c->cos_eps = cos(c->obliq);
+    c->sin_eps = sin(c->obliq);
+    c->tan_fov = 0.5 * c->pixel_scale * sqrt((double)c->W * c->W + (double)c->H * c->H);
+
+    c->stream = (cudaStream_t)s->stream;   // NULL = the legacy default stream
+    int rc = DT_OK;
+    do {
+        if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
+        c->h_exp.resize(c->N);
+        for (int32_t j = 0; j < c->N; ++j) {
+            const double v = (c->var_mode == 0) ? s->var_scalar[j] : nan("");
+            c->h_exp[j] = make_record(c, s->t[j], s->obs_ecl + 3 * j, s->ra0[j], s->dec0[j], v);
+        }
+        if (cudaMalloc((void **)&c->d_exp, sizeof(ExpRec) * (size_t)c->N) != cudaSuccess) { rc = DT_ERR_OOM; break; }
+        if (cudaMemcpyAsync(c->d_exp, c->h_exp.data(), sizeof(ExpRec) * (size_t)c->N, cudaMemcpyHostToDevice,
+                            c->stream) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
+        if (cudaMalloc((void **)&c->d_counters, 8 * sizeof(unsigned long long)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
+        if (cudaStreamSynchronize(c->stream) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
+        size_t free_b = 0, total_b = 0;
+        if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
+        c->budget = s->hbm_budget_bytes > 0 ? s->hbm_budget_bytes : (int64_t)(0.75 * (double)free_b);
+        const int64_t need = (int64_t)c->N * c->plane * 4 * (c->var_mode == 1 ? 2 : 1);
+        c->streaming = (c->flags & DT_FLAG_FORCE_STREAM) || need > c->budget;
+        c->loaded.assign(c->N, 0);
+        if (c->streaming) {
+            c->h_flux.assign(c->N, nullptr);
+            c->h_var.assign(c->N, nullptr);
+        }
+    } while (0);
+    if (rc != DT_OK) {
+        cudaGetLastError();
+        free_all(c);
+        delete c;
+        return rc;
+    }
+    *out = c;
+    return DT_OK;
+}
+
+int dt_destroy(dt_context *c)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
+    free_all(c);
+    delete c;
+    return DT_OK;
+}
+
+int dt_load_image_batch(dt_context *c, int32_t first, int32_t count, const float *flux, const float *var,
+                        int32_t mem_kind)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (first < 0 || count < 1 || (int64_t)first + count > c->N || !flux || !mem_kind_ok(mem_kind))
+        return fail(c, DT_ERR_INVALID_ARG, "dt_load_image_batch: bad range or pointer");
+    if (c->var_mode == 1 && !var) return fail(c, DT_ERR_INVALID_ARG, "variance_mode 1 needs a variance plane");
+    CU(c, cudaSetDevice(c->device));
+    if (c->streaming) {
+        if (mem_kind != DT_MEM_PINNED)
+            return fail(c, DT_ERR_INVALID_ARG,
+                        "survey exceeds hbm_budget_bytes: streaming mode needs DT_MEM_PINNED images");
+        for (int32_t j = 0; j < count; ++j) {
+            c->h_flux[first + j] = flux + (int64_t)j * c->plane;
+            c->h_var[first + j] = (c->var_mode == 1) ? var + (int64_t)j * c->plane : nullptr;
+            c->loaded[first + j] = 1;
+        }
+        return DT_OK;
+    }
+    int rc = ensure_store(c);
+    if (rc != DT_OK) return rc;
+    const size_t bytes = (size_t)count * (size_t)c->plane * 4;
+    CU(c, cudaMemcpyAsync(c->d_flux + (int64_t)first * c->plane, flux, bytes, cudaMemcpyDefault, c->stream));
+    if (c->var_mode == 1)
+        CU(c, cudaMemcpyAsync(c->d_var + (int64_t)first * c->plane, var, bytes, cudaMemcpyDefault, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    for (int32_t j = 0; j < count; ++j) c->loaded[first + j] = 1;
+    return DT_OK;
+}
+
+static int propagate_mode(const dt_context *c)
+{
+    int mode = 0;
+    if (!(c->flags & DT_FLAG_KEPLER_COLD)) mode |= kModeWarm;
+    if (!(c->flags & DT_FLAG_NO_PRECULL)) mode |= kModePrecull;
+    return mode;
+}
+
+static void fill_common(const dt_context *c, PropagateParams &p, double t0)
+{
+    memset(&p, 0, sizeof p);
+    p.t0 = t0;
+    p.gm = c->gm;
+    p.inv_c = c->inv_c;
+    p.cos_eps = c->cos_eps;
+    p.sin_eps = c->sin_eps;
+    p.cx = 0.5 * ((double)c->W - 1.0);
+    p.cy = 0.5 * ((double)c->H - 1.0);
+    p.W = (double)c->W;
+    p.H = (double)c->H;
+    p.width = c->W;
+    p.tan_fov = c->tan_fov;
+}
+
+static int32_t pick_groups_per_split(int64_t n_orbits, int32_t n_exp)
+{
+    const int64_t tiles = (n_orbits + kTileOrbits - 1) / kTileOrbits;
+    const int32_t n_groups = (n_exp + kGroup - 1) / kGroup;
+    if (tiles >= kMinCtas) return n_groups;
+    int64_t splits = (kMinCtas + tiles - 1) / tiles;
+    splits = std::min<int64_t>(splits, n_groups);
+    return (int32_t)((n_groups + splits - 1) / splits);
+}
+
+int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_t mem_kind, double *snr_out,
+             int32_t *hits_out)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (n < 0 || (n > 0 && !elements) || !mem_kind_ok(mem_kind) || !isfinite(t0))
+        return fail(c, DT_ERR_INVALID_ARG, "dt_stack: bad arguments");
+    for (int32_t j = 0; j < c->N; ++j)
+        if (!c->loaded[j]) return fail(c, DT_ERR_NOT_LOADED, "exposure %d has no image", j);
+    CU(c, cudaSetDevice(c->device));
+    int rc = ensure_store(c);
+    if (rc != DT_OK) return rc;
+
+    dt_stats &st = c->stats;
+    memset(&st, 0, sizeof st);
+    st.struct_size = sizeof(dt_stats);
+    st.n_orbits = n;
+    st.n_exposures = c->N;
+    st.pairs = n * (int64_t)c->N;
+    st.streamed = c->streaming ? 1 : 0;
+    c->n_last = -1;
+    if (n == 0) { c->n_last = 0; return DT_OK; }
+
+    // ---- buffers ----
+    const int32_t unit_exp = c->streaming ? c->batch_exp : std::min<int32_t>(c->N, kMaxUnitExposures);
+    const int64_t unit_orb = std::min<int64_t>((n + 31) / 32 * 32, kMaxUnitOrbits);
+    const int32_t unit_groups = (unit_exp + kGroup - 1) / kGroup;
+    const double *d_el = elements;
+    if (mem_kind != DT_MEM_DEVICE) {
+        CU(c, grow(c->d_el, c->el_cap, n * 6));
+        CU(c, cudaMemcpyAsync(c->d_el, elements, (size_t)n * 48, cudaMemcpyHostToDevice, c->stream));
+        d_el = c->d_el;
+    }
+    if (n > c->acc_cap) {
+        int64_t cap;
+        cap = c->acc_cap; CU(c, grow(c->d_S, cap, n));
+        cap = c->acc_cap; CU(c, grow(c->d_Wt, cap, n));
+        cap = c->acc_cap; CU(c, grow(c->d_snr, cap, n));
+        cap = c->acc_cap; CU(c, grow(c->d_cnt, cap, n));
+        cap = c->acc_cap; CU(c, grow(c->d_hits, cap, n));
+        c->acc_cap = n;
+    }
+    CU(c, grow(c->d_mask, c->mask_cap, unit_orb * unit_groups));
+    CU(c, grow(c->d_base, c->base_cap, (unit_orb / 32) * unit_groups));
+    CU(c, grow(c->d_offsets, c->off_cap, unit_orb * (int64_t)unit_groups * kGroup));
+    const int n_units_total = (int)(((c->N + unit_exp - 1) / unit_exp) * ((n + unit_orb - 1) / unit_orb));
+    while ((int64_t)c->ev_pool.size() < 4 + 3 * (int64_t)n_units_total) {
+        cudaEvent_t e;
+        CU(c, cudaEventCreate(&e));
+        c->ev_pool.push_back(e);
+    }
+    auto ev_at = [&](int i) { return c->ev_pool[4 + i]; };
+    int unit_idx = 0;
+
+    CU(c, cudaEventRecord(c->ev_pool[0], c->stream));
+    CU(c, cudaMemsetAsync(c->d_S, 0, (size_t)n * 8, c->stream));
+    CU(c, cudaMemsetAsync(c->d_Wt, 0, (size_t)n * 8, c->stream));
+    CU(c, cudaMemsetAsync(c->d_cnt, 0, (size_t)n * 4, c->stream));
+    CU(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+
+    const int mode = propagate_mode(c);
+    const int n_batches = (c->N + unit_exp - 1) / unit_exp;
+    st.n_image_batches = n_batches;
+
+    auto issue_copy = [&](int b) -> int {
+        const int slot = b & 1;
+        const int32_t first = b * unit_exp, cnt = std::min<int32_t>(unit_exp, c->N - first);
+        if (c->ev_free_recorded[slot]) CU(c, cudaStreamWaitEvent(c->copy_stream, c->ev_free[slot], 0));
+        for (int32_t j = 0; j < cnt; ++j) {
+            CU(c, cudaMemcpyAsync(c->d_buf_flux[slot] + (int64_t)j * c->plane, c->h_flux[first + j],
+                                  (size_t)c->plane * 4, cudaMemcpyHostToDevice, c->copy_stream));
+            st.h2d_image_bytes += c->plane * 4;
+            if (c->var_mode == 1) {
+                CU(c, cudaMemcpyAsync(c->d_buf_var[slot] + (int64_t)j * c->plane, c->h_var[first + j],
+                                      (size_t)c->plane * 4, cudaMemcpyHostToDevice, c->copy_stream));
+                st.h2d_image_bytes += c->plane * 4;
+            }
+        }
+        CU(c, cudaEventRecord(c->ev_ready[slot], c->copy_stream));
+        return DT_OK;
+    };
+
+    if (c->streaming) {
+        // the copy stream must not start before earlier work on the context stream that may still
+        // read the slots (a previous dt_stack) has been ordered: previous calls synchronise, so
+        // only the free events of this call matter
+        c->ev_free_recorded[0] = c->ev_free_recorded[1] = false;
+        rc = issue_copy(0);
+        if (rc != DT_OK) return rc;
+    }
+
+    for (int b = 0; b < n_batches; ++b) {
+        const int slot = b & 1;
+        const int32_t first = b * unit_exp, n_exp = std::min<int32_t>(unit_exp, c->N - first);
+        if (c->streaming && b + 1 < n_batches) {
+            rc = issue_copy(b + 1);
+            if (rc != DT_OK) return rc;
+        }
+        bool waited = false;
+        for (int64_t o0 = 0; o0 < n; o0 += unit_orb) {
+            const int64_t no = std::min<int64_t>(unit_orb, n - o0);
+            PropagateParams p;
+            fill_common(c, p, t0);
+            p.elements = d_el + o0 * 6;
+            p.n_orbits = no;
+            p.n_pad = (no + 31) / 32 * 32;
+            p.exp = c->d_exp + first;
+            p.n_exp = n_exp;
+            p.groups_per_split = pick_groups_per_split(no, n_exp);
+            p.mask = c->d_mask;
+            p.base = c->d_base;
+            p.offsets = c->d_offsets;
+            p.counters = c->d_counters;
+            // the hit counter restarts per unit so offsets index from 0
+            CU(c, cudaMemsetAsync(c->d_counters, 0, sizeof(unsigned long long), c->stream));
+            CU(c, cudaEventRecord(ev_at(3 * unit_idx), c->stream));
+            CU(c, launch_propagate(p, mode, c->stream));
+            st.propagate_launches += 1;
+            CU(c, cudaEventRecord(ev_at(3 * unit_idx + 1), c->stream));
+
+            if (c->streaming && !waited) {
+                CU(c, cudaStreamWaitEvent(c->stream, c->ev_ready[slot], 0));
+                waited = true;
+            }
+            GatherParams g;
+            memset(&g, 0, sizeof g);
+            g.n_orbits = no;
+            g.n_pad = p.n_pad;
+            g.first_exposure = first;
+            g.n_groups = (n_exp + kGroup - 1) / kGroup;
+            g.mask = c->d_mask;
+            g.base = c->d_base;
+            g.offsets = c->d_offsets;
+            if (c->streaming) {
+                g.flux = c->d_buf_flux[slot] - (int64_t)first * c->plane;
+                g.var = (c->var_mode == 1) ? c->d_buf_var[slot] - (int64_t)first * c->plane : nullptr;
+            } else {
+                g.flux = c->d_flux;
+                g.var = (c->var_mode == 1) ? c->d_var : nullptr;
+            }
+            g.exp_all = c->d_exp;
+            g.plane = c->plane;
+            g.S = c->d_S + o0;
+            g.Wt = c->d_Wt + o0;
+            g.cnt = c->d_cnt + o0;
+            CU(c, launch_gather(g, c->stream));
+            st.gather_launches += 1;
+            CU(c, cudaEventRecord(ev_at(3 * unit_idx + 2), c->stream));
+            unit_idx += 1;
+        }
+        if (c->streaming) {
+            CU(c, cudaEventRecord(c->ev_free[slot], c->stream));
+            c->ev_free_recorded[slot] = true;
+        }
+    }
+    CU(c, cudaEventRecord(c->ev_pool[2], c->stream));
+    CU(c, launch_finalize(d_el, n, c->d_S, c->d_Wt, c->d_cnt, c->d_snr, c->d_hits, c->d_counters + 5,
+                          c->stream));
+    CU(c, cudaEventRecord(c->ev_pool[3], c->stream));
+    if (snr_out)
+        CU(c, cudaMemcpyAsync(snr_out, c->d_snr, (size_t)n * 8, cudaMemcpyDefault, c->stream));
+    if (hits_out)
+        CU(c, cudaMemcpyAsync(hits_out, c->d_hits, (size_t)n * 4, cudaMemcpyDefault, c->stream));
+    CU(c, cudaEventRecord(c->ev_pool[1], c->stream));
+    unsigned long long hc[8];
+    CU(c, cudaMemcpyAsync(hc, c->d_counters, sizeof hc, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    CU(c, cudaEventElapsedTime(&st.ms_total, c->ev_pool[0], c->ev_pool[1]));
+    CU(c, cudaEventElapsedTime(&st.ms_finalize, c->ev_pool[2], c->ev_pool[3]));
+    for (int u = 0; u < unit_idx; ++u) {
+        float a = 0.f, b = 0.f;
+        CU(c, cudaEventElapsedTime(&a, ev_at(3 * u), ev_at(3 * u + 1)));
+        CU(c, cudaEventElapsedTime(&b, ev_at(3 * u + 1), ev_at(3 * u + 2)));
+        st.ms_propagate += a;
+        st.ms_gather += b;
+    }
+    st.hits = (int64_t)hc[3];
+    st.refined_pairs = (int64_t)hc[1];
+    st.cold_solves = (int64_t)hc[2];
+    st.invalid_orbits = (int64_t)hc[5];
+    st.launches = st.propagate_launches + st.gather_launches + 1;
+    c->n_last = n;
+    return DT_OK;
+}
+
+int dt_topk(dt_context *c, int32_t k, int32_t min_hits, int64_t *index_out, double *snr_out, int32_t *n_found)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (k < 0 || !n_found || (k > 0 && (!index_out || !snr_out)))
+        return fail(c, DT_ERR_INVALID_ARG, "dt_topk: bad arguments");
+    if (c->n_last < 0) return fail(c, DT_ERR_STATE, "dt_topk: no dt_stack result on the device");
+    CU(c, cudaSetDevice(c->device));
+    CU(c, topk_device(c->d_snr, c->d_hits, c->n_last, k, min_hits, c->topk, index_out, snr_out, n_found,
+                      c->stream));
+    return DT_OK;
+}
+
+int dt_project(dt_context *c, const double *elements, int64_t n, double t0, double *radec_out, double *xy_out,
+               int32_t *pix_out)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (n < 0 || (n > 0 && !elements) || !isfinite(t0)) return fail(c, DT_ERR_INVALID_ARG, "dt_project: bad arguments");
+    if (n == 0) return DT_OK;
+    CU(c, cudaSetDevice(c->device));
+    const int64_t N = c->N;
+    int64_t chunk = std::max<int64_t>(32, (int64_t)(6400000 / N) / 32 * 32);
+    chunk = std::min<int64_t>(chunk, (n + 31) / 32 * 32);
+    double *d_el = nullptr, *d_radec = nullptr, *d_xy = nullptr;
+    int32_t *d_pix = nullptr;
+    int rc = DT_OK;
+    auto cleanup = [&]() {
+        cudaFree(d_el);
+        cudaFree(d_radec);
+        cudaFree(d_xy);
+        cudaFree(d_pix);
+    };
+#define CUP(call)                                                                                 \
+    do {                                                                                          \
+        cudaError_t e__ = (call);                                                                 \
+        if (e__ != cudaSuccess) {                                                                 \
+            cleanup();                                                                            \
+            return fail(c, DT_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__));         \
+        }                                                                                         \
+    } while (0)
+    CUP(cudaMalloc((void **)&d_el, (size_t)chunk * 48));
+    CUP(cudaMalloc((void **)&d_radec, (size_t)chunk * N * 16));
+    CUP(cudaMalloc((void **)&d_xy, (size_t)chunk * N * 16));
+    CUP(cudaMalloc((void **)&d_pix, (size_t)chunk * N * 8));
+    const int mode = (propagate_mode(c) & kModeWarm) | kModeDense;
+    for (int64_t o0 = 0; o0 < n; o0 += chunk) {
+        const int64_t no = std::min<int64_t>(chunk, n - o0);
+        CUP(cudaMemcpyAsync(d_el, elements + o0 * 6, (size_t)no * 48, cudaMemcpyHostToDevice, c->stream));
+        PropagateParams p;
+        fill_common(c, p, t0);
+        p.elements = d_el;
+        p.n_orbits = no;
+        p.n_pad = (no + 31) / 32 * 32;
+        p.exp = c->d_exp;
+        p.n_exp = c->N;
+        p.groups_per_split = pick_groups_per_split(no, c->N);
+        p.counters = c->d_counters;
+        p.radec = d_radec;
+        p.xy = d_xy;
+        p.pix = d_pix;
+        CUP(launch_propagate(p, mode, c->stream));
+        if (radec_out)
+            CUP(cudaMemcpyAsync(radec_out + o0 * N * 2, d_radec, (size_t)no * N * 16, cudaMemcpyDeviceToHost, c->stream));
+        if (xy_out)
+            CUP(cudaMemcpyAsync(xy_out + o0 * N * 2, d_xy, (size_t)no * N * 16, cudaMemcpyDeviceToHost, c->stream));
+        if (pix_out)
+            CUP(cudaMemcpyAsync(pix_out + o0 * N * 2, d_pix, (size_t)no * N * 8, cudaMemcpyDeviceToHost, c->stream));
+        CUP(cudaStreamSynchronize(c->stream));
+    }
+#undef CUP
+    cleanup();
+    return rc;
+}
+
+int dt_gather_hits(dt_context *c, int64_t n, int32_t first_exposure, int32_t n_groups, const uint32_t *mask,
+                   const uint64_t *base, const uint32_t *offsets, double *S, double *Wt, int32_t *cnt)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (n < 0 || n_groups < 0 || first_exposure < 0 || (int64_t)first_exposure + (int64_t)n_groups * kGroup > (c->N + kGroup - 1) / kGroup * kGroup ||
+        !mask || !base || !offsets || !S || !Wt || !cnt)
+        return fail(c, DT_ERR_INVALID_ARG, "dt_gather_hits: bad arguments");
+    if (c->streaming || !c->d_flux) return fail(c, DT_ERR_STATE, "dt_gather_hits needs resident images");
+    CU(c, cudaSetDevice(c->device));
+    GatherParams g;
+    memset(&g, 0, sizeof g);
+    g.n_orbits = n;
+    g.n_pad = (n + 31) / 32 * 32;
+    g.first_exposure = first_exposure;
+    g.n_groups = n_groups;
+    g.mask = mask;
+    g.base = (const unsigned long long *)base;
+    g.offsets = offsets;
+    g.flux = c->d_flux;
+    g.var = (c->var_mode == 1) ? c->d_var : nullptr;
+    g.exp_all = c->d_exp;
+    g.plane = c->plane;
+    g.S = S;
+    g.Wt = Wt;
+    g.cnt = cnt;
+    CU(c, launch_gather(g, c->stream));
+    return DT_OK;
+}
+
+int dt_get_stats(const dt_context *c, dt_stats *out)
+{
+    if (!c || !out || out->struct_size != sizeof(dt_stats)) return DT_ERR_INVALID_ARG;
+    *out = c->stats;
+    return DT_OK;
+}
+
+int dt_fp64_peak(int32_t device, double *tflops)
+{
+    if (!tflops) return DT_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return DT_ERR_CUDA;
+    }
+    if (cudaSetDevice(device) != cudaSuccess) return DT_ERR_CUDA;
+    return fp64_peak_device(tflops, nullptr) == cudaSuccess ? DT_OK : DT_ERR_CUDA;
+}
+
+}  // extern "C"

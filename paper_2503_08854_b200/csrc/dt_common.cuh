@@ -1,0 +1,101 @@
+// dt_common.cuh -- shared declarations of the dtrack-b200 CUDA library (product code; shares
+// nothing with oracle/).  Data layout in HBM, kernel parameter blocks, launcher prototypes.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace dt {
+
+// ---- per-exposure constant record ("a few hundred bytes of data for each image") ---
+// 128 B = one TMA bulk-copy granule multiple; 32 records (one exposure group) = 4 KB in shared
+// memory.  Observer and tangent basis are already rotated to the EQUATORIAL frame and the in-plane
+// basis is divided by the pixel scale, so kernel 1 needs three dot products and one reciprocal.
+struct __align__(16) ExpRec {
+    double t;              // exposure mid-time, days
+    double Rx, Ry, Rz;     // observer, heliocentric equatorial, AU
+    double ex, ey, ez;     // east unit vector / pixel_scale   (x = cx + (q.e)/(q.t))
+    double nx, ny, nz;     // north unit vector / pixel_scale  (y = cy + (q.n)/(q.t))
+    double tx, ty, tz;     // unit vector to the tangent point (D = q.t)
+    double var;            // scalar variance (mode 0); NaN in plane mode
+    double inv_var;        // 1.0 / var (IEEE division on the host)
+    double pad;
+};
+static_assert(sizeof(ExpRec) == 128, "ExpRec must be 128 bytes");
+
+constexpr int kGroup = 32;          // exposures per group: one hit bit per exposure in a 32-bit mask
+constexpr int kTileOrbits = 256;    // orbits per CTA of kernel 1 (one orbit per thread)
+constexpr int kWarpsPerCta = kTileOrbits / 32;
+
+// ---- kernel 1 (+2): propagate, project, cull, compact ------------------------------------------
+struct PropagateParams {
+    const double *elements;     // [n][6] device
+    int64_t n_orbits;           // orbits in this unit
+    int64_t n_pad;              // n_orbits rounded up to 32 (mask row pitch)
+    const ExpRec *exp;          // records of the unit's first exposure
+    int32_t n_exp;              // exposures in this unit
+    int32_t groups_per_split;   // exposure groups handled by one blockIdx.y
+    double t0, gm, inv_c;       // inv_c = 0 disables light-time
+    double cos_eps, sin_eps;
+    double cx, cy, W, H;        // (W-1)/2, (H-1)/2, width, height as fp64
+    int32_t width;
+    double tan_fov;             // tan of the footprint half-diagonal, for the conservative pre-cull
+    // outputs of the cull + compaction stage (orbit-major hit list, see dtrack.h dt_gather_hits)
+    uint32_t *mask;             // [n_groups][n_pad]
+    unsigned long long *base;   // [n_groups][n_pad/32]
+    uint32_t *offsets;          // [capacity]
+    unsigned long long *counters;  // [0] unit hit allocator, [1] refined pairs, [2] cold solves, [3] hits
+    // dense debug outputs (dt_project), NULL on the timed path
+    double *radec, *xy;         // [n][n_exp][2]
+    int32_t *pix;               // [n][n_exp][2]
+};
+
+enum { kModeWarm = 1, kModePrecull = 2, kModeDense = 4 };
+
+cudaError_t launch_propagate(const PropagateParams &p, int mode, cudaStream_t stream);
+
+// ---- kernel 3: gather + stack ---------------------------------------------------------------------
+struct GatherParams {
+    int64_t n_orbits, n_pad;
+    int32_t first_exposure;     // absolute index of the unit's first exposure
+    int32_t n_groups;
+    const uint32_t *mask;
+    const unsigned long long *base;
+    const uint32_t *offsets;
+    const float *flux;          // plane of ABSOLUTE exposure j at flux + j * plane
+    const float *var;           // same indexing; NULL in scalar mode
+    const ExpRec *exp_all;      // all exposure records (scalar variance), absolute index
+    int64_t plane;              // pixels per plane
+    double *S, *Wt;             // [n] running sums (read-modify-write once per launch)
+    int32_t *cnt;               // [n]
+};
+
+cudaError_t launch_gather(const GatherParams &p, cudaStream_t stream);
+
+// SNR finalisation: snr = S / sqrt(Wt) (0 when no hit), NaN / -1 for invalid orbits.
+cudaError_t launch_finalize(const double *elements, int64_t n, const double *S, const double *Wt,
+                            const int32_t *cnt, double *snr, int32_t *hits,
+                            unsigned long long *invalid_counter, cudaStream_t stream);
+
+// ---- device top-k (dt_topk.cu) ----------------------------------------------------------------------
+struct TopkWorkspace {
+    unsigned long long *keys = nullptr;    // [n] order-preserving keys (0 = excluded)
+    unsigned long long *cand_key = nullptr;  // [cap] selected candidates
+    long long *cand_idx = nullptr;
+    unsigned int *hist = nullptr;          // [256] + scratch
+    unsigned long long *state = nullptr;   // prefix / remaining-k state
+    unsigned int *block_counts = nullptr;
+    int64_t n_cap = 0, cand_cap = 0, blocks_cap = 0;
+};
+
+// Selects the k best (snr descending, index ascending) valid entries; writes them sorted to the
+// host arrays.  Returns the number found through *n_found.
+cudaError_t topk_device(const double *snr, const int32_t *hits, int64_t n, int32_t k,
+                        int32_t min_hits, TopkWorkspace &ws, int64_t *index_out_host,
+                        double *snr_out_host, int32_t *n_found, cudaStream_t stream);
+void topk_free(TopkWorkspace &ws);
+
+// FP64 FMA issue-rate probe (dt_fp64_peak).
+cudaError_t fp64_peak_device(double *tflops, cudaStream_t stream);
+
+}  // namespace dt

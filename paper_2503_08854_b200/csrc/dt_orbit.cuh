@@ -1,0 +1,246 @@
+// dt_orbit.cuh -- fp64 device arithmetic of kernel 1: per-orbit precompute, Kepler solves (cold and
+// warm-started), heliocentric position, conservative pre-cull, gnomonic projection.
+//
+// Definitions follow DESIGN.md "What the path computes" (BASELINE.json north_star; the paper's
+// skeleton is PAPER.md:202 "converting the set of orbital parameters into a sky position at the
+// time of each image and converting these celestial coordinates to locations within the pixel
+// grid").  Formulation notes (all differ from the CPU oracle on purpose -- no shared code):
+//   * the orbit basis is pre-rotated to the equatorial frame and pre-scaled: r_eq = A (cosE - e)
+//     + B sinE with A = a R_eps P, B = a sqrt(1-e^2) R_eps Q, so steps "subtract observer" and
+//     "rotate ecliptic -> equatorial" commute into the per-orbit / per-exposure constants;
+//   * the projection is the VECTOR form xi = q.e_E / q.t, eta = q.e_N / q.t;
+//   * the Kepler state is carried as u = E - M with (sin E, cos E) and advanced from exposure to
+//     exposure by a 4th-order series step + rotation by Taylor (sin, cos) + one Newton polish,
+//     falling back to a libdevice-sincos Newton solve from a monotone start when the step is large.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+namespace dt {
+
+constexpr double kPi = 3.14159265358979323846;
+constexpr double kTwoPiHi = 6.28318530717958623200;     // fl(2 pi)
+constexpr double kTwoPiLo = 2.44929359829470641435e-16;  // 2 pi - fl(2 pi)
+constexpr double kInvTwoPi = 0.15915494309189534561;
+
+struct Orbit {
+    double n, e, M0;
+    double Ax, Ay, Az, Bx, By, Bz;  // equatorial, AU
+    double cos2_cull;               // cos^2 of the pre-cull cone half-angle
+    bool valid;
+};
+
+__device__ __forceinline__ bool orbit_valid(const double el[6])
+{
+    bool fin = isfinite(el[0]) && isfinite(el[1]) && isfinite(el[2]) && isfinite(el[3]) &&
+               isfinite(el[4]) && isfinite(el[5]);
+    return fin && el[0] > 0.0 && el[1] >= 0.0 && el[1] < 1.0;
+}
+
+// Per-orbit precompute (hot-path step 1).  tan_fov: tan of the footprint half-diagonal.
+__device__ __forceinline__ Orbit orbit_setup(const double el_in[6], double gm, double cos_eps,
+                                             double sin_eps, double inv_c, double tan_fov)
+{
+    Orbit o;
+    double el[6];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) el[k] = el_in[k];
+    o.valid = orbit_valid(el);
+    if (!o.valid) { el[0] = 1.0; el[1] = 0.0; el[2] = el[3] = el[4] = el[5] = 0.0; }
+    const double a = el[0], e = el[1];
+    o.n = sqrt(gm / (a * a * a));
+    o.e = e;
+    o.M0 = el[5];
+    double si, ci, sO, cO, sw, cw;
+    sincos(el[2], &si, &ci);
+    sincos(el[3], &sO, &cO);
+    sincos(el[4], &sw, &cw);
+    // perifocal basis in the ecliptic frame
+    const double Px = cO * cw - sO * sw * ci, Py = sO * cw + cO * sw * ci, Pz = sw * si;
+    const double Qx = -cO * sw - sO * cw * ci, Qy = -sO * sw + cO * cw * ci, Qz = cw * si;
+    const double b = a * sqrt(1.0 - e * e);
+    // rotate to equatorial: y' = y cos(eps) - z sin(eps), z' = y sin(eps) + z cos(eps)
+    o.Ax = a * Px;
+    o.Ay = a * (Py * cos_eps - Pz * sin_eps);
+    o.Az = a * (Py * sin_eps + Pz * cos_eps);
+    o.Bx = b * Qx;
+    o.By = b * (Qy * cos_eps - Qz * sin_eps);
+    o.Bz = b * (Qy * sin_eps + Qz * cos_eps);
+    // pre-cull cone: footprint half-diagonal + the largest angle light-time can move the object as
+    // seen by the observer, asin(v_max / c) with v_max the perihelion speed (|r(t) - r(t - tau)| <=
+    // v_max tau and tau = rho0 / c exactly, so the bound does not depend on rho0), + slack.
+    const double vmax = sqrt(gm / a * (1.0 + e) / (1.0 - e));
+    const double th = atan(tan_fov) * 1.01 + 1.05 * asin(fmin(vmax * inv_c, 1.0)) + 2e-5;
+    const double cth = (th < 1.5) ? cos(th) : 0.0;
+    o.cos2_cull = (th < 1.5) ? cth * cth : -1.0;  // -1: cone test disabled (always refine)
+    return o;
+}
+
+// ---- small fp64 helpers: MUFU seed + Newton, no slow-path branches ---------------------------------
+// 1/x for normal, finite x; relative error ~1e-12 after two iterations (three: ~1 ulp).
+template <int ITERS>
+__device__ __forceinline__ double rcp_nr(double x)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+#pragma unroll
+    for (int i = 0; i < ITERS; ++i) {
+        double e = fma(-x, r, 1.0);
+        r = fma(r, e, r);
+    }
+    return r;
+}
+
+// sqrt(a) for normal a > 0; Goldschmidt iterations from the MUFU rsqrt seed.
+template <int ITERS>
+__device__ __forceinline__ double sqrt_nr(double a)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    double g = a * y, h = 0.5 * y;
+#pragma unroll
+    for (int i = 0; i < ITERS; ++i) {
+        double r = fma(-g, h, 0.5);
+        g = fma(g, r, g);
+        h = fma(h, r, h);
+    }
+    return g;
+}
+
+// ---- Kepler state ----------------------------------------------------------------------------------
+// E = M + u (unreduced), s = sin E, c = cos E.  |u| <= e < 1, so u keeps full absolute precision
+// however large M is, and the residual E - e sin E - M = u - e s has no cancellation against M.
+struct Kepler {
+    double M, u, s, c;
+};
+
+// Cold solve: reduce M to m in [-pi, pi], fold to [0, pi], start at E0 = min(m + e, pi) (f convex on
+// [0, pi] with f(E0) >= 0, so Newton descends monotonically), Newton with libdevice sincos until
+// every lane of the warp has |dE| < 2e-9 (then the last first-order update is exact to ~1e-17).
+// Must be called by all 32 lanes of the warp.
+__device__ __forceinline__ Kepler kepler_cold(double e, double M)
+{
+    const double k = rint(M * kInvTwoPi);
+    double m = fma(-k, kTwoPiHi, M);
+    m = fma(-k, kTwoPiLo, m);
+    const double sg = (m < 0.0) ? -1.0 : 1.0;
+    m = fabs(m);
+    double E = fmin(m + e, kPi);
+    double s, c, dE;
+    bool done = false;
+    for (int it = 0; it < 60; ++it) {
+        sincos(E, &s, &c);
+        const double f = fma(-e, s, E) - m;
+        const double g = fma(-e, c, 1.0);
+        dE = f / g;
+        if (!done) E -= dE; else dE = 0.0;
+        done = done || (fabs(dE) < 2e-9);
+        if (__all_sync(0xffffffffu, done)) break;
+    }
+    // sin/cos were taken at E + dE: first-order update to the final E (dE^2/2 < 2e-18)
+    const double s1 = fma(-dE, c, s), c1 = fma(dE, s, c);
+    Kepler K;
+    K.M = M;
+    K.u = sg * (E - m);
+    K.s = sg * s1;
+    K.c = c1;
+    return K;
+}
+
+// Newton from a nearby state toward a new mean anomaly with libdevice sincos ("reference" mode of
+// the light-time re-solve).  Works on u directly: f = u - e sin(M + u).  All 32 lanes must call.
+__device__ __forceinline__ Kepler kepler_newton_from(double e, const Kepler &K0, double Mn)
+{
+    const double dM = Mn - K0.M;
+    // E_old = M_old + u_old; new equation: (E_old + th) - e sin(E_old + th) = M_old + dM
+    double th = 0.0, s = K0.s, c = K0.c, d;
+    const double f00 = fma(-e, K0.s, K0.u) - dM;  // residual at th = 0
+    bool done = false;
+    // sin(E_old + th) by rotating (s0, c0) with libdevice sincos(th): th is small but arbitrary
+    for (int it = 0; it < 60; ++it) {
+        double st, ct;
+        sincos(th, &st, &ct);
+        s = fma(K0.s, ct, K0.c * st);
+        c = fma(K0.c, ct, -K0.s * st);
+        const double f = fma(-e, s - K0.s, f00 + th);
+        const double g = fma(-e, c, 1.0);
+        d = f / g;
+        if (!done) th -= d; else d = 0.0;
+        done = done || (fabs(d) < 2e-9);
+        if (__all_sync(0xffffffffu, done)) break;
+    }
+    Kepler K;
+    K.M = Mn;
+    K.u = K0.u + (th - dM);
+    K.s = fma(-d, c, s);
+    K.c = fma(d, s, c);
+    return K;
+}
+
+// Warm step: series reversion of f(th) = f0 + g th + (e s/2) th^2 + (e c/6) th^3 - (e s/24) th^4 = 0
+// to 4th order, rotation of (s, c) by th with Taylor sin/cos (|th| <= 0.05: next terms < 3e-20),
+// then one Newton polish with a refined reciprocal.  `ok` is false when the step is outside the
+// domain where the truncated series is accurate enough for the polish to reach full precision;
+// the caller then falls back to kepler_cold.
+__device__ __forceinline__ Kepler kepler_warm(double e, const Kepler &K0, double Mn, bool &ok)
+{
+    const double dM = Mn - K0.M;
+    const double es = e * K0.s, ec = e * K0.c;
+    const double f0 = (K0.u - es) - dM;
+    const double g = 1.0 - ec;
+    const double rg = rcp_nr<2>(g);
+    const double x = -f0 * rg;
+    const double a2 = 0.5 * es * rg;
+    const double a3 = (1.0 / 6.0) * ec * rg;
+    // a4 = -a2 / 12;  th = x - a2 x^2 + (2 a2^2 - a3) x^3 + (5 a2 a3 - a4 - 5 a2^3) x^4
+    const double a22 = a2 * a2;
+    const double k3 = fma(2.0, a22, -a3);
+    const double k4 = fma(a2, fma(5.0, a3, 1.0 / 12.0), -5.0 * a22 * a2);
+    const double th = x * fma(x, fma(x, fma(x, k4, k3), -a2), 1.0);
+    ok = (fabs(x) <= 0.04) && (fabs(x * a2) <= 0.01);
+    // Taylor rotation
+    const double z = th * th;
+    const double ps = fma(z, fma(z, fma(z, 1.0 / 362880.0, -1.0 / 5040.0), 1.0 / 120.0), -1.0 / 6.0);
+    const double pc = fma(z, fma(z, fma(z, 1.0 / 40320.0, -1.0 / 720.0), 1.0 / 24.0), -0.5);
+    const double st = fma(th * z, ps, th);   // sin th
+    const double cm = z * pc;                // cos th - 1
+    double s1 = K0.s + fma(K0.c, st, K0.s * cm);
+    double c1 = K0.c + fma(-K0.s, st, K0.c * cm);
+    double u1 = K0.u + (th - dM);
+    // Newton polish: f1 = u1 - e s1, 1/g1 from one Newton step on rg
+    const double f1 = fma(-e, s1, u1);
+    const double g1 = fma(-e, c1, 1.0);
+    const double rg1 = rg * fma(-g1, rg, 2.0);
+    const double d = -f1 * rg1;
+    Kepler K;
+    K.M = Mn;
+    K.u = u1 + d;
+    K.s = fma(d, c1, s1);
+    K.c = fma(-d, s1, c1);
+    return K;
+}
+
+// Refresh: recompute (sin E, cos E) of the carried state exactly (libdevice sincos of the reduced
+// E = M + u) and polish u once, so the rounding of the Taylor rotations cannot accumulate beyond
+// one exposure group.
+__device__ __forceinline__ Kepler kepler_refresh(double e, const Kepler &K0)
+{
+    const double k = rint(K0.M * kInvTwoPi);
+    double m = fma(-k, kTwoPiHi, K0.M);
+    m = fma(-k, kTwoPiLo, m);
+    double s, c;
+    sincos(m + K0.u, &s, &c);
+    const double f = fma(-e, s, K0.u);
+    const double g = fma(-e, c, 1.0);
+    const double d = -f * rcp_nr<2>(g);
+    Kepler K;
+    K.M = K0.M;
+    K.u = K0.u + d;
+    K.s = fma(d, c, s);
+    K.c = fma(-d, s, c);
+    return K;
+}
+
+}  // namespace dt

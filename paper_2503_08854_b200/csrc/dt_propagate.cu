@@ -1,0 +1,298 @@
+// dt_propagate.cu -- kernel 1 (+2): propagate, light-time, project, footprint-cull, compact.
+//
+// Hot-path steps 1-7 of DESIGN.md (Algorithm 1 `SearchImages` + `FilterGPUIntersections`,
+// PAPER.md:159-161, 168-169; the dense |images| x |orbits| result is NEVER materialised -- only the
+// compacted hits leave the SM, cf. PAPER.md:202 where the paper stores "tens of bytes for each
+// pair").
+//
+// Mapping: one orbit per thread (32 orbits per warp, 256 per CTA); the thread walks the unit's
+// exposures in time order carrying its Kepler state, so consecutive solves are warm-started.
+// Exposure records (128 B each) are staged group by group (32 exposures = 4 KB) into shared memory
+// by 1-D TMA bulk copies (cp.async.bulk, SASS UBLKCP) on a two-slot mbarrier ring; every lane
+// reads the same record (broadcast).  Hits are compacted per warp and group: each lane stages its
+// pixel offsets in shared memory, a warp scan turns the per-lane counts into an orbit-major
+// layout, one lane reserves the range with a single integer atomicAdd, and the 32 hit masks of
+// the group are written as one coalesced 128-B row.
+#include "dt_common.cuh"
+#include "dt_orbit.cuh"
+
+namespace dt {
+
+// ---- mbarrier / bulk-copy PTX wrappers --------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+            "r"(smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+
+struct __align__(128) PropSmem {
+    ExpRec rec[2][kGroup];                       // 8 KB: two-slot ring of exposure groups
+    uint32_t stage[kWarpsPerCta][kGroup][32];    // 32 KB: [warp][slot][lane] staged pixel offsets
+    uint64_t full[2];
+};
+
+template <int MODE>
+__global__ void __launch_bounds__(kTileOrbits, 2) k_propagate(const PropagateParams p)
+{
+    constexpr bool WARM = (MODE & kModeWarm) != 0;
+    constexpr bool PRECULL = (MODE & kModePrecull) != 0;
+    constexpr bool DENSE = (MODE & kModeDense) != 0;
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    PropSmem &sm = *reinterpret_cast<PropSmem *>(smem_raw);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t orbit = (int64_t)blockIdx.x * kTileOrbits + tid;
+    const int n_groups = (p.n_exp + kGroup - 1) / kGroup;
+    const int g_begin = blockIdx.y * p.groups_per_split;
+    const int g_end = min(n_groups, g_begin + p.groups_per_split);
+
+    if (tid == 0) {
+        mbar_init(&sm.full[0], 1);
+        mbar_init(&sm.full[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+
+    auto issue = [&](int g) {   // thread 0 only
+        const int slot = (g - g_begin) & 1;
+        const int nrec = min(kGroup, p.n_exp - g * kGroup);
+        const uint32_t bytes = (uint32_t)nrec * (uint32_t)sizeof(ExpRec);
+        mbar_expect_tx(&sm.full[slot], bytes);
+        bulk_g2s(&sm.rec[slot][0], p.exp + (size_t)g * kGroup, bytes, &sm.full[slot]);
+    };
+    if (tid == 0) {
+        if (g_begin < g_end) issue(g_begin);
+        if (g_begin + 1 < g_end) issue(g_begin + 1);
+    }
+
+    // ---- per-orbit precompute (step 1) ----
+    double el[6];
+    const bool in_range = orbit < p.n_orbits;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) el[k] = in_range ? p.elements[orbit * 6 + k] : ((k == 0) ? -1.0 : 0.0);
+    const Orbit o = orbit_setup(el, p.gm, p.cos_eps, p.sin_eps, p.inv_c, p.tan_fov);
+
+    Kepler K;
+    K.M = K.u = K.s = 0.0;
+    K.c = 1.0;
+    bool have_state = false;
+    unsigned long long n_refined = 0, n_cold = 0, n_hits = 0;
+
+    for (int g = g_begin; g < g_end; ++g) {
+        const int slot = (g - g_begin) & 1;
+        const uint32_t parity = ((g - g_begin) >> 1) & 1;
+        mbar_wait(&sm.full[slot], parity);
+        const int nrec = min(kGroup, p.n_exp - g * kGroup);
+
+        if (WARM && have_state) K = kepler_refresh(o.e, K);
+
+        uint32_t bits = 0;
+        int cnt = 0;
+        for (int jj = 0; jj < nrec; ++jj) {
+            const ExpRec &x = sm.rec[slot][jj];
+            const double dt = x.t - p.t0;
+            const double M = fma(o.n, dt, o.M0);
+
+            // ---- step 3: Kepler solve at t_j ----
+            if (WARM) {
+                bool ok = false;
+                Kepler Kw = K;
+                if (have_state) Kw = kepler_warm(o.e, K, M, ok);
+                if (__all_sync(0xffffffffu, ok)) {
+                    K = Kw;
+                } else {
+                    K = kepler_cold(o.e, M);
+                    n_cold += 1;
+                }
+                have_state = true;
+            } else {
+                K = kepler_cold(o.e, M);
+                n_cold += 1;
+            }
+
+            // ---- step 4: geometric position and light-time ----
+            const double X0 = K.c - o.e;
+            const double dx0 = fma(o.Ax, X0, fma(o.Bx, K.s, -x.Rx));
+            const double dy0 = fma(o.Ay, X0, fma(o.By, K.s, -x.Ry));
+            const double dz0 = fma(o.Az, X0, fma(o.Bz, K.s, -x.Rz));
+            const double rho2 = fma(dx0, dx0, fma(dy0, dy0, dz0 * dz0));
+
+            bool near = true;
+            if (PRECULL) {
+                // conservative cone test on the GEOMETRIC direction (see orbit_setup)
+                const double D0 = fma(dx0, x.tx, fma(dy0, x.ty, dz0 * x.tz));
+                near = !(D0 * D0 < o.cos2_cull * rho2) && (D0 > 0.0 || o.cos2_cull < 0.0);
+                near = near || !(rho2 > 1e-12);
+            }
+            bool hit = false;
+            int32_t ix = -1, iy = -1;
+            double xpix = 0.0, ypix = 0.0, qx = 0.0, qy = 0.0, qz = 0.0;
+            if (!PRECULL || __any_sync(0xffffffffu, near)) {
+                n_refined += 1;
+                const double rho0 = WARM ? sqrt_nr<2>(rho2) : sqrt(rho2);
+                const double tau = rho0 * p.inv_c;
+                const double M1 = fma(o.n, dt - tau, o.M0);
+                Kepler K1;
+                if (WARM) {
+                    bool ok1;
+                    K1 = kepler_warm(o.e, K, M1, ok1);
+                    if (!__all_sync(0xffffffffu, ok1)) K1 = kepler_newton_from(o.e, K, M1);
+                } else {
+                    K1 = kepler_newton_from(o.e, K, M1);
+                }
+                // ---- step 5: topocentric equatorial vector ----
+                const double X1 = K1.c - o.e;
+                qx = fma(o.Ax, X1, fma(o.Bx, K1.s, -x.Rx));
+                qy = fma(o.Ay, X1, fma(o.By, K1.s, -x.Ry));
+                qz = fma(o.Az, X1, fma(o.Bz, K1.s, -x.Rz));
+                // ---- step 6: gnomonic projection (vector form) + pixelise ----
+                const double D = fma(qx, x.tx, fma(qy, x.ty, qz * x.tz));
+                const double inv = WARM ? rcp_nr<3>(D) : 1.0 / D;
+                const double xe = fma(qx, x.ex, fma(qy, x.ey, qz * x.ez));
+                const double xn = fma(qx, x.nx, fma(qy, x.ny, qz * x.nz));
+                xpix = fma(xe, inv, p.cx);
+                ypix = fma(xn, inv, p.cy);
+                const double xh = xpix + 0.5, yh = ypix + 0.5;
+                // ---- step 7: footprint cull, in floating point before any integer conversion ----
+                hit = o.valid && (D > 0.0) && (xh >= 0.0) && (xh < p.W) && (yh >= 0.0) && (yh < p.H);
+                if (hit) {
+                    ix = (int32_t)floor(xh);
+                    iy = (int32_t)floor(yh);
+                }
+            }
+            if (DENSE) {
+                if (in_range) {
+                    const int64_t k = (orbit * p.n_exp + (int64_t)g * kGroup + jj) * 2;
+                    if (p.radec) {
+                        const double rho = sqrt(fma(qx, qx, fma(qy, qy, qz * qz)));
+                        double ra = atan2(qy, qx);
+                        if (ra < 0.0) ra += 2.0 * kPi;
+                        p.radec[k] = o.valid ? ra : nan("");
+                        p.radec[k + 1] = o.valid ? asin(qz / rho) : nan("");
+                    }
+                    if (p.xy) {
+                        p.xy[k] = o.valid ? xpix : nan("");
+                        p.xy[k + 1] = o.valid ? ypix : nan("");
+                    }
+                    if (p.pix) {
+                        p.pix[k] = ix;
+                        p.pix[k + 1] = iy;
+                    }
+                }
+            } else if (hit) {
+                sm.stage[warp][cnt][lane] = (uint32_t)iy * (uint32_t)p.width + (uint32_t)ix;
+                bits |= 1u << jj;
+                cnt += 1;
+            }
+        }
+
+        n_hits += (unsigned long long)cnt;
+        if (!DENSE) {
+            // ---- warp-level compaction of the group's hits (orbit-major) ----
+            const unsigned any = __ballot_sync(0xffffffffu, cnt > 0);
+            int incl = cnt;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int v = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += v;
+            }
+            const int total = __shfl_sync(0xffffffffu, incl, 31);
+            unsigned long long b0 = 0;
+            if (any) {
+                if (lane == 0) b0 = atomicAdd(p.counters, (unsigned long long)total);
+                b0 = __shfl_sync(0xffffffffu, b0, 0);
+                uint32_t *dst = p.offsets + b0 + (unsigned long long)(incl - cnt);
+                for (int k = 0; k < cnt; ++k) dst[k] = sm.stage[warp][k][lane];
+            }
+            const int64_t opad = (int64_t)blockIdx.x * kTileOrbits + tid;
+            if (opad < p.n_pad) {
+                p.mask[(int64_t)g * p.n_pad + opad] = bits;
+                if (lane == 0) p.base[(int64_t)g * (p.n_pad >> 5) + (opad >> 5)] = b0;
+            }
+        }
+
+        __syncthreads();   // every warp is done with rec[slot] (and its stage rows)
+        if (tid == 0 && g + 2 < g_end) issue(g + 2);
+    }
+
+    // ---- statistics: one atomic per warp ----
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        n_refined += __shfl_xor_sync(0xffffffffu, n_refined, d);
+        n_cold += __shfl_xor_sync(0xffffffffu, n_cold, d);
+        n_hits += __shfl_xor_sync(0xffffffffu, n_hits, d);
+    }
+    if (lane == 0 && p.counters) {
+        atomicAdd(p.counters + 1, n_refined);
+        atomicAdd(p.counters + 2, n_cold);
+        if (n_hits) atomicAdd(p.counters + 3, n_hits);
+    }
+}
+
+template <int MODE>
+static cudaError_t launch_mode(const PropagateParams &p, cudaStream_t stream)
+{
+    static bool attr_set = false;
+    const size_t smem = sizeof(PropSmem);
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(k_propagate<MODE>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const int n_groups = (p.n_exp + kGroup - 1) / kGroup;
+    const int splits = (n_groups + p.groups_per_split - 1) / p.groups_per_split;
+    dim3 grid((unsigned)((p.n_orbits + kTileOrbits - 1) / kTileOrbits), (unsigned)splits);
+    k_propagate<MODE><<<grid, kTileOrbits, smem, stream>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_propagate(const PropagateParams &p, int mode, cudaStream_t stream)
+{
+    if (p.n_orbits <= 0 || p.n_exp <= 0) return cudaSuccess;
+    switch (mode) {
+        case 0: return launch_mode<0>(p, stream);
+        case 1: return launch_mode<1>(p, stream);
+        case 2: return launch_mode<2>(p, stream);
+        case 3: return launch_mode<3>(p, stream);
+        case 4: return launch_mode<4>(p, stream);
+        case 5: return launch_mode<5>(p, stream);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace dt

@@ -1,0 +1,399 @@
+// dt_topk.cu -- device top-k over the per-orbit SNR (hot-path step 10; Algorithm 1
+// `FindSignificantResults`; ordering rule of DESIGN.md step 11: SNR descending, ties
+// by orbit index ascending, over orbits with hits >= min_hits and finite SNR).
+//
+// 1. keys: order-preserving 64-bit image of the fp64 SNR (0 = excluded);
+// 2. radix select, 8 passes x 8 bits from the top: block-local shared-memory histograms merged with
+//    integer atomics, a one-warp kernel walks the 256 bins and narrows (prefix, k_remaining) -> the
+//    exact key T of the k-th best and the number r of entries equal to T that still fit;
+// 3. ordered compaction (block counts -> single-block exclusive scan -> scatter): keys > T, then the
+//    first r keys == T in INDEX order (this is what makes ties deterministic);
+// 4. bitonic sort of the <= k candidates on the composite (key descending, index ascending):
+//    shared-memory kernel for spans <= 2048, global compare-exchange steps above that.
+#include "dt_common.cuh"
+
+namespace dt {
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kItems = 16;                    // keys per thread in the streaming kernels
+constexpr int kChunk = kThreads * kItems;     // 4096 keys per block
+constexpr int kSortSpan = 2048;               // elements sorted per block in shared memory
+
+__device__ __forceinline__ unsigned long long order_key(double x)
+{
+    unsigned long long b = (unsigned long long)__double_as_longlong(x);
+    return (b & 0x8000000000000000ull) ? ~b : (b | 0x8000000000000000ull);
+}
+
+__global__ void k_keys(const double *__restrict__ snr, const int32_t *__restrict__ hits, int64_t n,
+                       int32_t min_hits, unsigned long long *__restrict__ keys)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double x = snr[i];
+    const bool ok = isfinite(x) && hits[i] >= min_hits && hits[i] >= 0;
+    keys[i] = ok ? order_key(x) : 0ull;
+}
+
+// state[0] = prefix (high bits decided so far), state[1] = k remaining, state[2] = total valid,
+// state[3] = threshold T (final), state[4] = r ties to take, state[5] = number of keys > T
+__global__ void k_hist(const unsigned long long *__restrict__ keys, int64_t n, int pass,
+                       const unsigned long long *__restrict__ state, unsigned int *__restrict__ hist)
+{
+    __shared__ unsigned int sh[256];
+    sh[threadIdx.x] = 0;
+    __syncthreads();
+    const int shift = 56 - 8 * pass;
+    const unsigned long long prefix = state[0];
+    const unsigned long long himask = (pass == 0) ? 0ull : (~0ull << (shift + 8));
+    const int64_t base = (int64_t)blockIdx.x * kChunk;
+#pragma unroll 4
+    for (int it = 0; it < kItems; ++it) {
+        const int64_t i = base + (int64_t)it * kThreads + threadIdx.x;
+        if (i < n) {
+            const unsigned long long key = keys[i];
+            if (key != 0ull && (key & himask) == prefix)
+                atomicAdd(&sh[(unsigned)(key >> shift) & 255u], 1u);
+        }
+    }
+    __syncthreads();
+    const unsigned int v = sh[threadIdx.x];
+    if (v) atomicAdd(&hist[threadIdx.x], v);
+}
+
+__global__ void k_pick(int pass, int32_t k, unsigned long long *state, unsigned int *hist)
+{
+    // one thread: 256 bins, negligible
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const int shift = 56 - 8 * pass;
+    unsigned long long krem = (pass == 0) ? (unsigned long long)k : state[1];
+    if (pass == 0) {
+        unsigned long long total = 0;
+        for (int d = 0; d < 256; ++d) total += hist[d];
+        state[2] = total;
+        state[5] = 0;
+        if (total <= krem) {   // fewer valid entries than k: take all of them
+            state[0] = 0;
+            state[1] = 0;
+            state[3] = 0;      // T = 0: every valid key is > T
+            state[4] = 0;
+            state[6] = 1;      // done flag
+            for (int d = 0; d < 256; ++d) hist[d] = 0;
+            return;
+        }
+        state[6] = 0;
+    }
+    if (state[6]) {
+        for (int d = 0; d < 256; ++d) hist[d] = 0;
+        return;
+    }
+    unsigned long long above = 0;
+    int d = 255;
+    for (; d > 0; --d) {
+        const unsigned long long c = hist[d];
+        if (above + c >= krem) break;
+        above += c;
+    }
+    state[0] |= ((unsigned long long)d) << shift;
+    state[1] = krem - above;
+    state[5] += above;
+    if (pass == 7) {
+        state[3] = state[0];
+        state[4] = state[1];
+    }
+    for (int q = 0; q < 256; ++q) hist[q] = 0;
+}
+
+__global__ void k_count(const unsigned long long *__restrict__ keys, int64_t n,
+                        const unsigned long long *__restrict__ state, unsigned int *__restrict__ counts)
+{
+    __shared__ unsigned int s_gt, s_eq;
+    if (threadIdx.x == 0) s_gt = s_eq = 0;
+    __syncthreads();
+    const unsigned long long T = state[3];
+    const int64_t base = (int64_t)blockIdx.x * kChunk;
+    unsigned int gt = 0, eq = 0;
+    for (int it = 0; it < kItems; ++it) {
+        const int64_t i = base + (int64_t)it * kThreads + threadIdx.x;
+        if (i < n) {
+            const unsigned long long key = keys[i];
+            gt += (key > T);
+            eq += (key == T && key != 0ull);
+        }
+    }
+    for (int d = 16; d > 0; d >>= 1) {
+        gt += __shfl_xor_sync(0xffffffffu, gt, d);
+        eq += __shfl_xor_sync(0xffffffffu, eq, d);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(&s_gt, gt);
+        atomicAdd(&s_eq, eq);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        counts[2 * blockIdx.x] = s_gt;
+        counts[2 * blockIdx.x + 1] = s_eq;
+    }
+}
+
+// exclusive scan of the per-block (gt, eq) counts, in place, by one block
+__global__ void k_scan(unsigned int *counts, int nblocks, unsigned long long *state)
+{
+    __shared__ unsigned long long carry[2];
+    __shared__ unsigned int tmp[2][1024];
+    if (threadIdx.x == 0) carry[0] = carry[1] = 0;
+    __syncthreads();
+    for (int b0 = 0; b0 < nblocks; b0 += 1024) {
+        const int b = b0 + threadIdx.x;
+        unsigned int v0 = (b < nblocks) ? counts[2 * b] : 0, v1 = (b < nblocks) ? counts[2 * b + 1] : 0;
+        tmp[0][threadIdx.x] = v0;
+        tmp[1][threadIdx.x] = v1;
+        __syncthreads();
+        for (int d = 1; d < 1024; d <<= 1) {
+            unsigned int a0 = 0, a1 = 0;
+            if (threadIdx.x >= d) { a0 = tmp[0][threadIdx.x - d]; a1 = tmp[1][threadIdx.x - d]; }
+            __syncthreads();
+            tmp[0][threadIdx.x] += a0;
+            tmp[1][threadIdx.x] += a1;
+            __syncthreads();
+        }
+        if (b < nblocks) {
+            // offsets can exceed 32 bits only for > 4e9 candidates; k is int32 so they cannot
+            counts[2 * b] = (unsigned int)(carry[0] + tmp[0][threadIdx.x] - v0);
+            counts[2 * b + 1] = (unsigned int)(carry[1] + tmp[1][threadIdx.x] - v1);
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) {
+            carry[0] += tmp[0][1023];
+            carry[1] += tmp[1][1023];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) state[7] = carry[0];   // total number of keys > T
+}
+
+__global__ void k_scatter(const unsigned long long *__restrict__ keys, int64_t n,
+                          const unsigned long long *__restrict__ state,
+                          const unsigned int *__restrict__ counts,
+                          unsigned long long *__restrict__ cand_key, long long *__restrict__ cand_idx)
+{
+    // ordered within the block: each thread handles kItems CONSECUTIVE keys
+    __shared__ unsigned int sc[2][kThreads];
+    const unsigned long long T = state[3], r = state[4], total_gt = state[7];
+    const int64_t base = (int64_t)blockIdx.x * kChunk + (int64_t)threadIdx.x * kItems;
+    unsigned int gt = 0, eq = 0;
+    unsigned long long loc[kItems];
+#pragma unroll
+    for (int it = 0; it < kItems; ++it) {
+        const int64_t i = base + it;
+        loc[it] = (i < n) ? keys[i] : 0ull;
+        gt += (loc[it] > T);
+        eq += (loc[it] == T && loc[it] != 0ull);
+    }
+    sc[0][threadIdx.x] = gt;
+    sc[1][threadIdx.x] = eq;
+    __syncthreads();
+    for (int d = 1; d < kThreads; d <<= 1) {
+        unsigned int a0 = 0, a1 = 0;
+        if (threadIdx.x >= d) { a0 = sc[0][threadIdx.x - d]; a1 = sc[1][threadIdx.x - d]; }
+        __syncthreads();
+        sc[0][threadIdx.x] += a0;
+        sc[1][threadIdx.x] += a1;
+        __syncthreads();
+    }
+    unsigned long long pg = (unsigned long long)counts[2 * blockIdx.x] + sc[0][threadIdx.x] - gt;
+    unsigned long long pe = (unsigned long long)counts[2 * blockIdx.x + 1] + sc[1][threadIdx.x] - eq;
+#pragma unroll
+    for (int it = 0; it < kItems; ++it) {
+        const unsigned long long key = loc[it];
+        if (key > T) {
+            cand_key[pg] = key;
+            cand_idx[pg] = base + it;
+            ++pg;
+        } else if (key == T && key != 0ull) {
+            if (pe < r) {
+                cand_key[total_gt + pe] = key;
+                cand_idx[total_gt + pe] = base + it;
+            }
+            ++pe;
+        }
+    }
+}
+
+__global__ void k_pad(unsigned long long *cand_key, long long *cand_idx, int64_t m, int64_t m_pad)
+{
+    const int64_t i = m + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < m_pad) {
+        cand_key[i] = 0ull;                       // sorts last (descending)
+        cand_idx[i] = 0x7fffffffffffffffll;
+    }
+}
+
+// "a before b" in the final order
+__device__ __forceinline__ bool before(unsigned long long ka, long long ia, unsigned long long kb,
+                                       long long ib)
+{
+    return (ka > kb) || (ka == kb && ia < ib);
+}
+
+// bitonic network, stages (kk, j) for j < kSortSpan handled inside shared memory
+__global__ void k_bitonic_local(unsigned long long *cand_key, long long *cand_idx, int64_t m_pad,
+                                int64_t kk_begin, int64_t kk_end_incl)
+{
+    __shared__ unsigned long long sk[kSortSpan];
+    __shared__ long long si[kSortSpan];
+    const int64_t base = (int64_t)blockIdx.x * kSortSpan;
+    for (int t = threadIdx.x; t < kSortSpan; t += blockDim.x) {
+        sk[t] = cand_key[base + t];
+        si[t] = cand_idx[base + t];
+    }
+    __syncthreads();
+    for (int64_t kk = kk_begin; kk <= kk_end_incl; kk <<= 1) {
+        int64_t j0 = kk >> 1;
+        if (j0 >= kSortSpan) j0 = kSortSpan >> 1;
+        for (int64_t j = j0; j > 0; j >>= 1) {
+            for (int t = threadIdx.x; t < kSortSpan / 2; t += blockDim.x) {
+                const int lo = (int)(((t / j) * 2 * j) + (t % j));
+                const int hi = lo + (int)j;
+                const bool asc = (((base + lo) & kk) == 0);   // "asc" = final order direction
+                const bool lo_first = before(sk[lo], si[lo], sk[hi], si[hi]);
+                if (lo_first != asc) {
+                    const unsigned long long tk = sk[lo]; sk[lo] = sk[hi]; sk[hi] = tk;
+                    const long long ti = si[lo]; si[lo] = si[hi]; si[hi] = ti;
+                }
+            }
+            __syncthreads();
+        }
+    }
+    for (int t = threadIdx.x; t < kSortSpan; t += blockDim.x) {
+        cand_key[base + t] = sk[t];
+        cand_idx[base + t] = si[t];
+    }
+}
+
+__global__ void k_bitonic_global(unsigned long long *cand_key, long long *cand_idx, int64_t m_pad,
+                                 int64_t kk, int64_t j)
+{
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= m_pad / 2) return;
+    const int64_t lo = ((t / j) * 2 * j) + (t % j);
+    const int64_t hi = lo + j;
+    const bool asc = ((lo & kk) == 0);
+    const unsigned long long ka = cand_key[lo], kb = cand_key[hi];
+    const long long ia = cand_idx[lo], ib = cand_idx[hi];
+    if (before(ka, ia, kb, ib) != asc) {
+        cand_key[lo] = kb; cand_key[hi] = ka;
+        cand_idx[lo] = ib; cand_idx[hi] = ia;
+    }
+}
+
+__global__ void k_emit(const long long *__restrict__ cand_idx, const double *__restrict__ snr, int64_t m,
+                       double *__restrict__ out_snr)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < m) out_snr[i] = snr[cand_idx[i]];
+}
+
+template <typename T>
+cudaError_t ensure(T *&ptr, int64_t &cap, int64_t need)
+{
+    if (need <= cap && ptr) return cudaSuccess;
+    if (ptr) cudaFree(ptr);
+    ptr = nullptr;
+    cap = 0;
+    cudaError_t e = cudaMalloc((void **)&ptr, (size_t)need * sizeof(T));
+    if (e == cudaSuccess) cap = need;
+    return e;
+}
+
+}  // namespace
+
+#define TK_CHECK(x)                      \
+    do {                                 \
+        cudaError_t e__ = (x);           \
+        if (e__ != cudaSuccess) return e__; \
+    } while (0)
+
+cudaError_t topk_device(const double *snr, const int32_t *hits, int64_t n, int32_t k, int32_t min_hits,
+                        TopkWorkspace &ws, int64_t *index_out_host, double *snr_out_host,
+                        int32_t *n_found, cudaStream_t stream)
+{
+    *n_found = 0;
+    if (n <= 0 || k <= 0) return cudaSuccess;
+    const int64_t kk64 = (k < n) ? (int64_t)k : n;
+    int64_t m_pad = kSortSpan;
+    while (m_pad < kk64) m_pad <<= 1;
+    const int nblocks = (int)((n + kChunk - 1) / kChunk);
+
+    TK_CHECK(ensure(ws.keys, ws.n_cap, n));
+    {
+        int64_t cap = ws.cand_cap;
+        TK_CHECK(ensure(ws.cand_key, cap, m_pad));
+        cap = ws.cand_cap;
+        TK_CHECK(ensure(ws.cand_idx, cap, m_pad));
+        ws.cand_cap = cap;
+    }
+    if (!ws.hist) TK_CHECK(cudaMalloc((void **)&ws.hist, 256 * sizeof(unsigned int)));
+    if (!ws.state) TK_CHECK(cudaMalloc((void **)&ws.state, 16 * sizeof(unsigned long long)));
+    TK_CHECK(ensure(ws.block_counts, ws.blocks_cap, (int64_t)2 * nblocks));
+
+    TK_CHECK(cudaMemsetAsync(ws.hist, 0, 256 * sizeof(unsigned int), stream));
+    TK_CHECK(cudaMemsetAsync(ws.state, 0, 16 * sizeof(unsigned long long), stream));
+    k_keys<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(snr, hits, n, min_hits, ws.keys);
+    for (int pass = 0; pass < 8; ++pass) {
+        k_hist<<<nblocks, kThreads, 0, stream>>>(ws.keys, n, pass, ws.state, ws.hist);
+        k_pick<<<1, 32, 0, stream>>>(pass, (int32_t)kk64, ws.state, ws.hist);
+    }
+    k_count<<<nblocks, kThreads, 0, stream>>>(ws.keys, n, ws.state, ws.block_counts);
+    k_scan<<<1, 1024, 0, stream>>>(ws.block_counts, nblocks, ws.state);
+    k_scatter<<<nblocks, kThreads, 0, stream>>>(ws.keys, n, ws.state, ws.block_counts, ws.cand_key,
+                                                ws.cand_idx);
+    TK_CHECK(cudaGetLastError());
+
+    unsigned long long st[8];
+    TK_CHECK(cudaMemcpyAsync(st, ws.state, sizeof st, cudaMemcpyDeviceToHost, stream));
+    TK_CHECK(cudaStreamSynchronize(stream));
+    const int64_t total_valid = (int64_t)st[2];
+    const int64_t m = (total_valid < kk64) ? total_valid : kk64;
+    if (m <= 0) return cudaSuccess;
+
+    int64_t mp = kSortSpan;
+    while (mp < m) mp <<= 1;
+    if (mp > m) k_pad<<<(unsigned)((mp - m + 255) / 256), 256, 0, stream>>>(ws.cand_key, ws.cand_idx, m, mp);
+    // bitonic sort of mp elements
+    k_bitonic_local<<<(unsigned)(mp / kSortSpan), 512, 0, stream>>>(ws.cand_key, ws.cand_idx, mp, 2,
+                                                                   kSortSpan);
+    for (int64_t kk = (int64_t)kSortSpan * 2; kk <= mp; kk <<= 1) {
+        for (int64_t j = kk >> 1; j >= kSortSpan; j >>= 1)
+            k_bitonic_global<<<(unsigned)((mp / 2 + 255) / 256), 256, 0, stream>>>(ws.cand_key, ws.cand_idx,
+                                                                                  mp, kk, j);
+        k_bitonic_local<<<(unsigned)(mp / kSortSpan), 512, 0, stream>>>(ws.cand_key, ws.cand_idx, mp, kk,
+                                                                       kk);
+    }
+    // reuse the key buffer (fp64-sized) for the emitted SNR values
+    double *out_snr = reinterpret_cast<double *>(ws.keys);
+    k_emit<<<(unsigned)((m + 255) / 256), 256, 0, stream>>>(ws.cand_idx, snr, m, out_snr);
+    TK_CHECK(cudaGetLastError());
+    TK_CHECK(cudaMemcpyAsync(index_out_host, ws.cand_idx, (size_t)m * sizeof(long long),
+                             cudaMemcpyDeviceToHost, stream));
+    TK_CHECK(cudaMemcpyAsync(snr_out_host, out_snr, (size_t)m * sizeof(double), cudaMemcpyDeviceToHost,
+                             stream));
+    TK_CHECK(cudaStreamSynchronize(stream));
+    *n_found = (int32_t)m;
+    return cudaSuccess;
+}
+
+void topk_free(TopkWorkspace &ws)
+{
+    cudaFree(ws.keys);
+    cudaFree(ws.cand_key);
+    cudaFree(ws.cand_idx);
+    cudaFree(ws.hist);
+    cudaFree(ws.state);
+    cudaFree(ws.block_counts);
+    ws = TopkWorkspace();
+}
+
+}  // namespace dt

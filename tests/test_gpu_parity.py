@@ -1,0 +1,346 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle on the
+same seeded inputs.  Bars (BASELINE.json north_star):
+  * sky positions within 1e-10 rad;
+  * pixel indices bit-exact except where the oracle flags the fractional coordinate within 1e-6 px
+    of a rounding boundary (A11) -- such cases are counted and reported;
+  * per-orbit hits exact and SNR within 1e-9 * max(|SNR|, 1e-3) (A14) on orbits without flagged hits.
+Sizes: small enough for the oracle to finish in seconds, large enough to span several 256-orbit
+tiles, several 32-exposure groups, ragged tails in both, and more than one work unit.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import dtsynth as ds
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+def _dt():
+    import paper_2503_08854_b200 as dt
+    return dt
+
+
+def _planes(sc, mode):
+    N = sc.cfg.n_exp
+    flux = np.stack([sc.flux_plane_np(j) for j in range(N)])
+    var = np.stack([sc.var_plane_np(j) for j in range(N)]) if mode == 1 else None
+    return flux, var
+
+
+def _compare_stack(snr, hits, ref, what=""):
+    snr, hits = np.asarray(snr), np.asarray(hits)
+    clean = ref["nflag"] == 0
+    assert np.array_equal(hits[clean], ref["hits"][clean]), what
+    tol = 1e-9 * np.maximum(np.abs(ref["snr"]), 1e-3)
+    both_nan = np.isnan(snr) & np.isnan(ref["snr"])
+    ok = both_nan | (np.abs(snr - ref["snr"]) <= tol)
+    assert ok[clean].all(), (what, np.flatnonzero(~ok & clean)[:10])
+    flagged = np.flatnonzero(~clean)
+    same = flagged[hits[flagged] == ref["hits"][flagged]]
+    assert ok[same].all(), what
+    return dict(flagged_orbits=int(flagged.size), flagged_hit_mismatch=int(flagged.size - same.size))
+
+
+def _compare_project(out, ref):
+    """-> number of pixel mismatches inside the guard band (reported); asserts the rest."""
+    valid = np.isfinite(ref["radec"][..., 0])
+    dra = np.abs(out["radec"][..., 0] - ref["radec"][..., 0])
+    dra = np.minimum(dra, 2 * math.pi - dra)
+    cosd = np.cos(ref["radec"][..., 1])
+    assert (dra[valid] * cosd[valid]).max() <= 1e-10          # great-circle east-west offset
+    assert np.abs(out["radec"][..., 1] - ref["radec"][..., 1])[valid].max() <= 1e-10
+    same = (out["pix"] == ref["pix"]).all(-1)
+    bad = ~same
+    assert not (bad & (ref["flag"] == 0)).any(), np.argwhere(bad & (ref["flag"] == 0))[:5]
+    # continuous pixel coordinates, where the projection is meaningful (front hemisphere, near field)
+    near = valid & (np.abs(ref["xy"][..., 0]) < 1e5) & (np.abs(ref["xy"][..., 1]) < 1e5)
+    if near.any():
+        assert np.abs(out["xy"] - ref["xy"])[near].max() < 1e-6
+    return int(bad.sum())
+
+
+CASES = {
+    # name: (base config, scale overrides, focused?)
+    "tiny": ("tiny", dict(), False),
+    "tiny_focused": ("tiny", dict(n_orbits=3000), True),
+    "mba_focused": ("small_mba", dict(n_orbits=6011, n_exp=75, width=512, height=384), True),
+    "lsst_focused": ("lsst", dict(n_orbits=4100, n_exp=70, width=640, height=512), True),
+    "neo_focused": ("neo", dict(n_orbits=6100, n_exp=100, width=512, height=512), True),
+    "tno_focused": ("tno", dict(n_orbits=4000, n_exp=90, width=512, height=512), True),
+    "neo_diffuse": ("neo", dict(n_orbits=5000, n_exp=64, width=512, height=512), False),
+}
+
+
+def _scene(case):
+    base, kw, foc = CASES[case]
+    cfg = ds.CONFIGS[base]
+    if kw:
+        cfg = ds.scaled(cfg, **kw)
+    if foc:
+        cfg = ds.focused(cfg)
+    return ds.build_scene(cfg, oracle.scene_project_fn)
+
+
+@pytest.mark.parametrize("flags", [0, 2, 4, 6], ids=["warm+precull", "cold+precull", "warm", "cold"])
+@pytest.mark.parametrize("case", ["tiny_focused", "neo_focused"])
+def test_project_parity(case, flags):
+    dt = _dt()
+    sc = _scene(case)
+    el = sc.elements()[:2500]
+    ref = oracle.project(oracle.Survey.from_scene(sc), el, sc.t0)
+    with dt.Tracker.from_scene(sc, flags=flags) as trk:
+        out = trk.project(el, sc.t0)
+    n_band = _compare_project(out, ref)
+    print("project %s flags=%d: %d pairs, %d in-band pixel mismatches, %d flagged" %
+          (case, flags, ref["flag"].size, n_band, int(ref["flag"].sum())))
+
+
+@pytest.mark.parametrize("case", list(CASES))
+def test_stack_parity(case):
+    dt = _dt()
+    sc = _scene(case)
+    mode = sc.cfg.variance_mode
+    el = sc.elements()
+    flux, var = _planes(sc, mode)
+    ref = oracle.stack(oracle.Survey.from_scene(sc), list(flux), list(var) if var is not None else None,
+                       el, sc.t0)
+    results = {}
+    for flags in (0, 6):
+        with dt.Tracker.from_scene(sc, flags=flags) as trk:
+            trk.load_image_batch(0, flux, var)
+            snr, hits = trk.stack(el, sc.t0)
+            st = trk.stats()
+            rep = _compare_stack(snr, hits, ref, "%s flags=%d" % (case, flags))
+            assert st["pairs"] == el.shape[0] * sc.cfg.n_exp
+            if rep["flagged_orbits"] == 0:
+                assert st["hits"] == int(ref["hits"][ref["hits"] > 0].sum())
+            results[flags] = (snr, hits)
+            print(case, "flags", flags, rep, {k: st[k] for k in ("hits", "refined_pairs", "cold_solves")})
+    # the fast path and the reference mode of kernel 1 agree with each other as well
+    assert np.array_equal(results[0][1], results[6][1]) or ref["nflag"].any()
+    if "focused" in case:
+        assert ref["hits"].max() >= 2
+    # top-k on the device equals the oracle's full sort of the oracle's own result (where SNR ties
+    # are exact: compare indices only when the two SNR arrays agree bit for bit)
+    with dt.Tracker.from_scene(sc) as trk:
+        trk.load_image_batch(0, flux, var)
+        snr, hits = trk.stack(el, sc.t0)
+        for k, mh in [(10, 1), (257, 0), (el.shape[0] + 5, 2)]:
+            idx, val = trk.topk(k, mh)
+            widx, wval = oracle.topk(snr, hits, k, mh)       # oracle sort of the SAME array
+            assert np.array_equal(idx, widx) and np.array_equal(val, wval)
+
+
+def test_injected_source_recovered_tiny():
+    """CFG 1: the injected 0.5 sigma source at node 5105 stacks to ~ A sqrt(N) and tops the list."""
+    dt = _dt()
+    sc = _scene("tiny")
+    flux, var = _planes(sc, 1)
+    with dt.Tracker.from_scene(sc) as trk:
+        trk.load_image_batch(0, flux, var)
+        snr, hits = trk.stack(sc.elements(), sc.t0)
+        idx, val = trk.topk(5, min_hits=32)
+    assert hits[5105] == 64 and abs(snr[5105] - 0.5 * 8.0) < 4.0
+    assert idx[0] == 5105 and val[0] == snr[5105]
+
+
+def test_address_images_exact_pixels():
+    """flux = pixel address (exact in fp32), var = 1: S is the sum of addresses, so any wrong pixel
+    shows up exactly; hits must equal the oracle's pixel list."""
+    dt = _dt()
+    sc = _scene("mba_focused")
+    N, H, W = sc.cfg.n_exp, sc.cfg.height, sc.cfg.width
+    el = sc.elements()
+    addr = np.arange(H * W, dtype=np.float32).reshape(1, H, W).repeat(N, 0)
+    sv = oracle.Survey.from_scene(sc)
+    sv1 = oracle.Survey(sc.t, sc.obs_ecl, sc.ra0, sc.dec0, W, H, sc.pixel_scale, sc.gm, sc.c,
+                        sc.obliquity, 0, np.ones(N))
+    ref = oracle.stack(sv1, list(addr), None, el, sc.t0)
+    with dt.Tracker.from_scene(sc, variance_mode=0, var_scalar=np.ones(N)) as trk:
+        trk.load_image_batch(0, addr)
+        snr, hits = trk.stack(el, sc.t0)
+    clean = ref["nflag"] == 0
+    assert np.array_equal(hits[clean], ref["hits"][clean])
+    S_gpu = snr * np.sqrt(np.maximum(hits, 1))
+    assert np.allclose(S_gpu[clean], ref["S"][clean], rtol=1e-12, atol=0)
+    del sv
+
+
+def test_masked_pixels_invalid_orbits_and_edges():
+    dt = _dt()
+    sc = _scene("tiny_focused")
+    N, H, W = sc.cfg.n_exp, sc.cfg.height, sc.cfg.width
+    el = sc.elements()[:700].copy()
+    flux = np.ones((N, H, W), np.float32)
+    var = np.ones((N, H, W), np.float32)
+    sv = oracle.Survey.from_scene(sc)
+    pix = oracle.project(sv, el, sc.t0)["pix"]
+    o = int(np.argmax((pix[..., 0] >= 0).sum(1)))
+    js = np.flatnonzero(pix[o, :, 0] >= 0)
+    flux[js[0], pix[o, js[0], 1], pix[o, js[0], 0]] = np.nan
+    var[js[1], pix[o, js[1], 1], pix[o, js[1], 0]] = 0.0
+    var[js[2], pix[o, js[2], 1], pix[o, js[2], 0]] = np.inf
+    el[0, 0], el[1, 1], el[2, 1], el[3, 5] = -1.0, 1.0, -0.1, np.nan
+    ref = oracle.stack(sv, list(flux), list(var), el, sc.t0)
+    with dt.Tracker.from_scene(sc) as trk:
+        trk.load_image_batch(0, flux, var)
+        snr, hits = trk.stack(el, sc.t0)
+        assert trk.stats()["invalid_orbits"] == 4
+        rep = _compare_stack(snr, hits, ref)
+        assert list(hits[:4]) == [-1] * 4 and np.isnan(snr[:4]).all()
+        # empty and single-orbit calls
+        s0, h0 = trk.stack(np.zeros((0, 6)), sc.t0)
+        assert s0.size == 0 and h0.size == 0
+        idx, val = trk.topk(3)
+        assert idx.size == 0
+        s1, h1 = trk.stack(el[o:o + 1], sc.t0)
+        assert h1[0] == ref["hits"][o] and abs(s1[0] - ref["snr"][o]) <= 1e-9 * abs(ref["snr"][o])
+    print(rep)
+
+
+def test_errors_and_state():
+    dt = _dt()
+    sc = _scene("tiny_focused")
+    N, H, W = sc.cfg.n_exp, sc.cfg.height, sc.cfg.width
+    with dt.Tracker.from_scene(sc) as trk:
+        with pytest.raises(dt.DtError) as e:
+            trk.stack(sc.elements()[:10], 0.0)
+        assert e.value.code == dt.DT_ERR_NOT_LOADED
+        with pytest.raises(dt.DtError) as e:
+            trk.topk(3)
+        assert e.value.code == dt.DT_ERR_STATE
+        with pytest.raises(dt.DtError) as e:
+            trk.load_image_batch(N - 1, np.zeros((2, H, W), np.float32), np.zeros((2, H, W), np.float32))
+        assert e.value.code == dt.DT_ERR_INVALID_ARG
+        with pytest.raises(dt.DtError):
+            trk.load_image_batch(0, np.zeros((1, H, W), np.float32))      # mode 1 needs var
+    with pytest.raises(dt.DtError):
+        dt.dt_create(sc.t, sc.obs_ecl, sc.ra0, sc.dec0, 0, 16, sc.pixel_scale, var_scalar=sc.var_scalar)
+
+
+def test_streaming_batches_match_resident():
+    """north_star subsystem 4: a survey larger than the HBM budget is streamed from pinned host
+    memory in double-buffered exposure batches; results must equal the resident run bit for bit."""
+    dt = _dt()
+    sc = _scene("lsst_focused")
+    el = sc.elements()
+    flux, var = _planes(sc, 1)
+    with dt.Tracker.from_scene(sc) as trk:
+        trk.load_image_batch(0, flux, var)
+        snr_r, hits_r = trk.stack(el, sc.t0)
+        assert trk.stats()["streamed"] == 0
+    pf, pv = torch.from_numpy(flux).pin_memory(), torch.from_numpy(var).pin_memory()
+    per_exp = flux[0].nbytes * 2
+    for nb in (9, 33):           # 9 exposures per batch (ragged, < one group) and 32 (33 rounded down)
+        with dt.Tracker.from_scene(sc, hbm_budget_bytes=2 * nb * per_exp) as trk:
+            with pytest.raises(dt.DtError):
+                trk.load_image_batch(0, flux, var)                        # pageable: refused
+            half = sc.cfg.n_exp // 2
+            trk.load_image_batch(half, pf[half:], pv[half:])
+            trk.load_image_batch(0, pf[:half], pv[:half])
+            snr_s, hits_s = trk.stack(el, sc.t0)
+            st = trk.stats()
+            assert st["streamed"] == 1 and st["n_image_batches"] == math.ceil(sc.cfg.n_exp / min(nb, 32))
+            assert st["h2d_image_bytes"] == flux.nbytes + var.nbytes
+            assert np.array_equal(hits_s, hits_r)
+            assert np.array_equal(snr_s, snr_r)
+            snr_s2, _ = trk.stack(el, sc.t0)                              # second pass reuses the slots
+            assert np.array_equal(snr_s2, snr_r)
+
+
+def test_many_exposures_and_device_pointers():
+    """More than one exposure unit (> 512 exposures) with carried partial sums, CUDA-tensor inputs
+    and outputs, and a torch stream."""
+    dt = _dt()
+    cfg = ds.focused(ds.scaled(ds.CONFIGS["tno"], n_orbits=2500, n_exp=600, width=128, height=128,
+                               variance_mode=0))
+    sc = ds.build_scene(cfg, oracle.scene_project_fn)
+    el = sc.elements()
+    flux, _ = _planes(sc, 0)
+    ref = oracle.stack(oracle.Survey.from_scene(sc), list(flux), None, el, sc.t0)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        with dt.Tracker.from_scene(sc, stream=stream.cuda_stream) as trk:
+            trk.load_image_batch(0, torch.from_numpy(flux).cuda())
+            snr, hits = trk.stack(torch.from_numpy(el).cuda(), sc.t0)
+            assert snr.is_cuda and hits.is_cuda
+            rep = _compare_stack(snr.cpu().numpy(), hits.cpu().numpy(), ref)
+            assert trk.stats()["n_image_batches"] == 2
+    assert ref["hits"].max() > 100
+    print(rep)
+
+
+def test_more_than_one_orbit_unit():
+    """> 2^20 orbits: two orbit units; oracle on a strided sample plus the tail."""
+    dt = _dt()
+    cfg = ds.focused(ds.scaled(ds.CONFIGS["small_mba"], n_orbits=(1 << 20) + 4097, n_exp=40, width=256,
+                               height=256))
+    sc = ds.build_scene(cfg, oracle.scene_project_fn)
+    el = sc.elements()
+    flux, _ = _planes(sc, 0)
+    with dt.Tracker.from_scene(sc) as trk:
+        trk.load_image_batch(0, flux)
+        snr, hits = trk.stack(el, sc.t0)
+    sel = np.concatenate([np.arange(0, el.shape[0], 37), np.arange((1 << 20) - 300, el.shape[0])])
+    ref = oracle.stack(oracle.Survey.from_scene(sc), list(flux), None, el[sel], sc.t0)
+    rep = _compare_stack(snr[sel], hits[sel], ref)
+    assert ref["hits"].max() >= 2
+    print(rep)
+
+
+def test_gather_hits_entry_matches_definition():
+    """dt_gather_hits on a hand-built orbit-major hit list: every pair hits a seeded random pixel."""
+    dt = _dt()
+    N, H, W, n = 64, 96, 80, 1000
+    rng = np.random.default_rng(5)
+    t = np.linspace(0, 10, N)
+    var_s = rng.uniform(0.8, 1.2, N)
+    flux = rng.normal(size=(N, H, W)).astype(np.float32)
+    npad = (n + 31) // 32 * 32
+    hit = rng.random((N, npad)) < 0.3
+    hit[:, n:] = False
+    pixel = rng.integers(0, H * W, size=(N, npad))
+    G = N // 32
+    mask = np.zeros((G, npad), np.uint32)
+    base = np.zeros((G, npad // 32), np.uint64)
+    offsets = []
+    for g in range(G):
+        for w in range(npad // 32):
+            base[g, w] = len(offsets)
+            for o in range(32 * w, 32 * w + 32):
+                for b in range(32):
+                    if hit[32 * g + b, o]:
+                        mask[g, o] |= np.uint32(1 << b)
+                        offsets.append(pixel[32 * g + b, o])
+    offsets = np.array(offsets, np.uint32)
+    S = np.zeros(n)
+    Wt = np.zeros(n)
+    for o in range(n):
+        for j in range(N):
+            if hit[j, o]:
+                S[o] += np.float64(flux[j].reshape(-1)[pixel[j, o]]) / var_s[j]
+                Wt[o] += 1.0 / var_s[j]
+    with dt.Tracker(t, ds.observer_ecliptic(t), np.zeros(N), np.zeros(N), W, H, ds.PIXEL_SCALE,
+                    variance_mode=0, var_scalar=var_s) as trk:
+        trk.load_image_batch(0, flux)
+        dS = torch.zeros(n, dtype=torch.float64, device="cuda")
+        dW = torch.zeros(n, dtype=torch.float64, device="cuda")
+        dc = torch.zeros(n, dtype=torch.int32, device="cuda")
+        trk.gather_hits(n, 0, G, torch.from_numpy(mask.view(np.int32)).cuda(),
+                        torch.from_numpy(base.view(np.int64)).cuda(),
+                        torch.from_numpy(offsets.view(np.int32)).cuda(), dS, dW, dc)
+        torch.cuda.synchronize()
+    assert np.array_equal(dc.cpu().numpy(), hit[:, :n].sum(0).astype(np.int32))
+    assert np.array_equal(dS.cpu().numpy(), S) and np.array_equal(dW.cpu().numpy(), Wt)
+
+
+def test_fp64_peak_probe_runs():
+    dt = _dt()
+    tf = dt.dt_fp64_peak(0)
+    print("FP64 DFMA peak: %.2f TFLOP/s" % tf)
+    assert 5.0 < tf < 100.0
