@@ -48,6 +48,8 @@ def parse_args():
     ap.add_argument("--flags", type=int, default=0, help="dt_survey.flags (2: cold Kepler, 4: no pre-cull)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-gather-bench", action="store_true")
+    ap.add_argument("--gather-only", action="store_true", help="run only the kernel-3 micro-benchmarks")
     return ap.parse_args()
 
 
@@ -173,6 +175,61 @@ def run_reference(args, cfg, rank: int):
     print(json.dumps(line))
 
 
+# ---- kernel 3 micro-benchmarks (controlled hit lists over the workload's image set) ------
+GATHER_REGIMES = [
+    # name, cluster window (px), hit density per pair
+    ("L0_uniform_dense", 1 << 30, 1.0),
+    ("L0_uniform_sparse", 1 << 30, 0.05),
+    ("L1_clustered", 256, 1.0),
+    ("L2_reuse", 32, 1.0),
+]
+
+
+def gather_bench(dt, trk, cfg, dev, hbm_gbs, reps=5, regimes=None):
+    import torch
+    from dtsynth import hitlists
+    n = min(cfg.n_orbits, 1 << 20)
+    G = max(1, min(cfg.n_exp // 32, 15))
+    out = []
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    for name, cluster, density in (regimes or GATHER_REGIMES):
+        hl = hitlists.build(n, G, cfg.width, cfg.height, cluster, density, 7, dev)
+        S = torch.zeros(n, dtype=torch.float64, device=dev)
+        Wt = torch.zeros(n, dtype=torch.float64, device=dev)
+        cnt = torch.zeros(n, dtype=torch.int32, device=dev)
+        times = []
+        for r in range(reps + 2):
+            S.zero_(); Wt.zero_(); cnt.zero_()
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            trk.gather_hits(n, 0, G, hl["mask"], hl["base"], hl["offsets"], S, Wt, cnt)
+            e1.record()
+            torch.cuda.synchronize()
+            if r >= 2:
+                times.append(e0.elapsed_time(e1))
+        assert int(cnt.sum().item()) == hl["hits"]
+        ms = float(np.mean(times))
+        planes = 2 if cfg.variance_mode == 1 else 1
+        bytes_min = (hl["hits"] * 4 + hl["mask"].numel() * 4 + hl["base"].numel() * 8 +
+                     hl["unique_sectors"] * 32 * planes + hl["touched_orbits"] * 20)
+        gbs = bytes_min / (ms * 1e-3) * 1e-9
+        out.append({"regime": name, "hits": hl["hits"], "unique_sectors": hl["unique_sectors"],
+                    "bytes_min": int(bytes_min), "ms": ms, "hits_per_s": hl["hits"] / (ms * 1e-3),
+                    "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": gbs / hbm_gbs})
+        del hl, S, Wt, cnt
+        torch.cuda.empty_cache()
+    return out
+
+
+def measured_hbm_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    except Exception:
+        return 6650.0, "fallback 6.65 TB/s of B200_PROFILING.md (of fallback)"
+
+
 # ---- B200 arm ----------------------------------------------------------------------------------------------
 def main():
     args = parse_args()
@@ -223,6 +280,13 @@ def main():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    if args.gather_only:
+        hbm, src = measured_hbm_peak()
+        print(json.dumps({"gather_roofline": {"bound": "hbm", "kernel": "k_gather_stack", "peak_source": src,
+                                              "regimes": gather_bench(dt, trk, cfg, dev, hbm)}}))
+        trk.close()
+        return
 
     # ---- warm-up ----
     for _ in range(max(args.warmup, 3)):
@@ -306,6 +370,10 @@ def main():
                               "finalize": stats["ms_finalize"]},
                 "hits_per_step": int(stats["hits"]), "cold_solves": int(stats["cold_solves"]),
                 "wall_s_timed_region": wall}
+        if not args.no_gather_bench:
+            hbm, src = measured_hbm_peak()
+            line["gather_roofline"] = {"bound": "hbm", "kernel": "k_gather_stack", "peak_source": src,
+                                       "regimes": gather_bench(dt, trk, cfg, dev, hbm)}
         if not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(cfg)
         print(json.dumps(line))
