@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-gather-bench", action="store_true")
     ap.add_argument("--gather-only", action="store_true", help="run only the kernel-3 micro-benchmarks")
+    ap.add_argument("--gather-reps", type=int, default=5, help="timed repetitions per kernel-3 regime")
+    ap.add_argument("--gather-regimes", default="", help="comma-separated subset of the kernel-3 regimes")
     return ap.parse_args()
 
 
@@ -185,6 +187,13 @@ GATHER_REGIMES = [
 ]
 
 
+def pick_regimes(args):
+    if not args.gather_regimes:
+        return None
+    want = set(args.gather_regimes.split(","))
+    return [r for r in GATHER_REGIMES if r[0] in want]
+
+
 def gather_bench(dt, trk, cfg, dev, hbm_gbs, reps=5, regimes=None):
     import torch
     from dtsynth import hitlists
@@ -284,7 +293,8 @@ def main():
     if args.gather_only:
         hbm, src = measured_hbm_peak()
         print(json.dumps({"gather_roofline": {"bound": "hbm", "kernel": "k_gather_stack", "peak_source": src,
-                                              "regimes": gather_bench(dt, trk, cfg, dev, hbm)}}))
+                                              "regimes": gather_bench(dt, trk, cfg, dev, hbm, args.gather_reps,
+                                                                      pick_regimes(args))}}))
         trk.close()
         return
 
@@ -373,7 +383,8 @@ def main():
         if not args.no_gather_bench:
             hbm, src = measured_hbm_peak()
             line["gather_roofline"] = {"bound": "hbm", "kernel": "k_gather_stack", "peak_source": src,
-                                       "regimes": gather_bench(dt, trk, cfg, dev, hbm)}
+                                       "regimes": gather_bench(dt, trk, cfg, dev, hbm, args.gather_reps,
+                                                               pick_regimes(args))}
         if not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(cfg)
         print(json.dumps(line))
