@@ -212,7 +212,7 @@ def gather_bench(dt, trk, cfg, dev, hbm_gbs, reps=5, regimes=None):
             flush.fill_(1)
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
-            trk.gather_hits(n, 0, G, hl["mask"], hl["base"], hl["offsets"], S, Wt, cnt)
+            trk.gather_hits(n, 0, G, hl["mask"], hl["base"], hl["offsets"], hl["hits"], S, Wt, cnt)
             e1.record()
             torch.cuda.synchronize()
             if r >= 2:

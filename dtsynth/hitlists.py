@@ -1,6 +1,6 @@
 """Controlled hit lists for the kernel-3 (gather + stack) micro-benchmarks.
 
-Builds, on a CUDA device with torch, a hit list in the library's orbit-major format (see
+Builds, on a CUDA device with torch, a hit list in the library's hit-list format (see
 include/dtrack.h, dt_gather_hits) in which every (orbit, exposure) pair is a hit with probability
 `density` and the hit pixel is drawn uniformly from a `cluster` x `cluster` window whose centre
 moves from exposure to exposure:
@@ -34,22 +34,22 @@ def build(n_orbits: int, n_groups: int, width: int, height: int, cluster: int, d
             on = torch.rand((G, n_pad), device=device, generator=gen) < density
         on[:, n_orbits:] = False
         bits |= on.to(torch.int64) << b
-    cnt = torch.zeros((G, n_pad), dtype=torch.int64, device=device)
-    for b in range(32):
-        cnt += (bits >> b) & 1
-    start = torch.cumsum(cnt.reshape(-1), 0) - cnt.reshape(-1)           # orbit-major inside (g, tile)
-    base = start.reshape(G, tiles, 32)[:, :, 0].contiguous()
-    hits = int(cnt.sum().item())
-    # per hit: its exposure (ascending inside a lane's run) and a random pixel of the window
+    # hits of warp-tile w (32 consecutive orbits) in exposure (g, b): [G, tiles, 32]
+    cnt_gtb = torch.stack([((bits >> b) & 1).reshape(G, tiles, 32).sum(2) for b in range(32)], dim=2)
+    tile_tot = cnt_gtb.sum(2)                                            # [G, tiles]
+    base = (torch.cumsum(tile_tot.reshape(-1), 0) - tile_tot.reshape(-1)).reshape(G, tiles).contiguous()
+    seg = base.unsqueeze(2) + torch.cumsum(cnt_gtb, 2) - cnt_gtb         # start of exposure b's run
+    hits = int(tile_tot.sum().item())
+    # per hit: a random pixel of the window; block order = exposure-ascending, then lane-ascending
     offsets = torch.empty(max(hits, 1), dtype=torch.int32, device=device)
     sectors = 0
     cl = min(cluster, width, height)
     for g in range(G):
-        bg, sg, cg = bits[g], start.reshape(G, n_pad)[g], cnt[g]
-        rank = torch.zeros(n_pad, dtype=torch.int64, device=device)
+        bg = bits[g]
         sec_ids = []
         for b in range(32):
-            on = ((bg >> b) & 1).bool()
+            on2 = ((bg >> b) & 1).reshape(tiles, 32)
+            on = on2.bool().reshape(-1)
             k = int(on.sum().item())
             if k == 0:
                 continue
@@ -59,14 +59,15 @@ def build(n_orbits: int, n_groups: int, width: int, height: int, cluster: int, d
             px = cx + torch.randint(0, cl, (k,), device=device, generator=gen)
             py = cy + torch.randint(0, cl, (k,), device=device, generator=gen)
             off = py * width + px
-            pos = (sg + rank)[on]
+            lane_rank = torch.cumsum(on2, 1) - on2
+            pos = (seg[g, :, b].unsqueeze(1) + lane_rank).reshape(-1)[on]
             offsets[pos] = off.to(torch.int32)
-            rank += on.to(torch.int64)
             sec_ids.append(torch.unique((j * plane + off) >> 3))          # 8 fp32 per 32-B sector
         if sec_ids:
             sectors += int(sum(s.numel() for s in sec_ids))               # exposures are disjoint
+    cnt = tile_tot
     mask = (bits & 0xFFFFFFFF)
     mask = torch.where(mask >= (1 << 31), mask - (1 << 32), mask).to(torch.int32).contiguous()
-    touched = int((cnt.sum(0) > 0).sum().item())
+    touched = int((bits != 0).any(0).sum().item())
     return dict(mask=mask, base=base, offsets=offsets, hits=hits, unique_sectors=sectors,
                 touched_orbits=touched, n_pad=n_pad)

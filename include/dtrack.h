@@ -165,17 +165,20 @@ int dt_project(dt_context *ctx, const double *elements, int64_t n, double t0, do
 
 /*
  * dt_gather_hits: kernel 3 on a caller-supplied hit list (micro-benchmark / test entry).
- * The hit list uses the library's internal orbit-major format for ONE exposure range
+ * The hit list uses the library's internal format for ONE exposure range
  * [first_exposure, first_exposure + 32*n_groups): for group g and orbit o, bit b of
  * mask[g*n_pad + o] says orbit o hits exposure first_exposure + 32 g + b; the pixel offsets
- * (iy*W + ix) of warp-tile w = o/32 in group g start at offsets[base[g*(n_pad/32) + w]], orbit-major
- * then exposure-ascending.  n_pad = n rounded up to 32.  All pointers are DEVICE pointers.
+ * (iy*W + ix) of warp-tile w = o/32 in group g start at offsets[base[g*(n_pad/32) + w]] and are
+ * ordered exposure-ascending, then orbit-ascending inside the tile (so the hits of one exposure
+ * are contiguous).  n_pad = n rounded up to 32; n <= 2^20, n_groups <= 16, fewer than 2^32 hits.
+ * n_hits = number of entries of `offsets` (the kernel picks its dense lock-step or its sparse
+ * schedule from the hit density).  All pointers are DEVICE pointers.
  * Accumulates into S[n], Wt[n] (fp64) and cnt[n] (int32), which the caller zero-initialises.
  * Images must be resident (DT_ERR_STATE in streaming mode).
  */
 int dt_gather_hits(dt_context *ctx, int64_t n, int32_t first_exposure, int32_t n_groups,
-                   const uint32_t *mask, const uint64_t *base, const uint32_t *offsets, double *S,
-                   double *Wt, int32_t *cnt);
+                   const uint32_t *mask, const uint64_t *base, const uint32_t *offsets,
+                   int64_t n_hits, double *S, double *Wt, int32_t *cnt);
 
 int dt_get_stats(const dt_context *ctx, dt_stats *out);
 const char *dt_last_error(const dt_context *ctx);

@@ -75,7 +75,7 @@ def lib():
         L.dt_stack.argtypes = [vp, vp, C.c_int64, C.c_double, C.c_int32, vp, vp]
         L.dt_topk.argtypes = [vp, C.c_int32, C.c_int32, C.POINTER(C.c_int64), dp, ip]
         L.dt_project.argtypes = [vp, dp, C.c_int64, C.c_double, dp, dp, ip]
-        L.dt_gather_hits.argtypes = [vp, C.c_int64, C.c_int32, C.c_int32, vp, vp, vp, vp, vp, vp]
+        L.dt_gather_hits.argtypes = [vp, C.c_int64, C.c_int32, C.c_int32, vp, vp, vp, C.c_int64, vp, vp, vp]
         L.dt_get_stats.argtypes = [vp, C.POINTER(dt_stats)]
         L.dt_last_error.argtypes = [vp]
         L.dt_last_error.restype = C.c_char_p
@@ -196,13 +196,14 @@ def dt_project(ctx, elements, t0: float, n_exposures: int):
     return dict(radec=radec, xy=xy, pix=pix)
 
 
-def dt_gather_hits(ctx, n: int, first_exposure: int, n_groups: int, mask, base, offsets, S, Wt, cnt) -> None:
+def dt_gather_hits(ctx, n: int, first_exposure: int, n_groups: int, mask, base, offsets, n_hits: int, S, Wt,
+                   cnt) -> None:
     """Kernel 3 on a caller-built hit list; all arguments are torch CUDA tensors (see dtrack.h)."""
     for x in (mask, base, offsets, S, Wt, cnt):
         if not (_is_torch(x) and x.is_cuda and x.is_contiguous()):
             raise ValueError("dt_gather_hits takes contiguous CUDA tensors")
     _check(lib().dt_gather_hits(ctx, n, first_exposure, n_groups, mask.data_ptr(), base.data_ptr(),
-                                offsets.data_ptr(), S.data_ptr(), Wt.data_ptr(), cnt.data_ptr()), ctx)
+                                offsets.data_ptr(), n_hits, S.data_ptr(), Wt.data_ptr(), cnt.data_ptr()), ctx)
 
 
 def dt_get_stats(ctx) -> dict:
@@ -246,8 +247,8 @@ class Tracker:
     def project(self, elements, t0=0.0):
         return dt_project(self.ctx, elements, t0, self.n_exposures)
 
-    def gather_hits(self, n, first_exposure, n_groups, mask, base, offsets, S, Wt, cnt):
-        dt_gather_hits(self.ctx, n, first_exposure, n_groups, mask, base, offsets, S, Wt, cnt)
+    def gather_hits(self, n, first_exposure, n_groups, mask, base, offsets, n_hits, S, Wt, cnt):
+        dt_gather_hits(self.ctx, n, first_exposure, n_groups, mask, base, offsets, n_hits, S, Wt, cnt)
 
     def stats(self):
         return dt_get_stats(self.ctx)

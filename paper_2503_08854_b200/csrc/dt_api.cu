@@ -7,6 +7,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -64,6 +65,10 @@ struct dt_context {
     uint32_t *d_offsets = nullptr;
     int64_t mask_cap = 0, base_cap = 0, off_cap = 0;
     unsigned long long *d_counters = nullptr;           // [8]
+    int *d_progress = nullptr;                          // kernel 3 lock-step counters, one per exposure of a unit
+    int32_t gather_window = 1;                          // exposures the slowest and fastest CTA may be apart
+    int32_t gather_lockstep = -1;                       // -1: decided on the device from the hit density
+    int32_t gather_ld_cached = 1;
     std::vector<cudaEvent_t> ev_pool;                   // timing events
 
     TopkWorkspace topk;
@@ -129,6 +134,7 @@ void free_all(dt_context *c)
     cudaFree(c->d_base);
     cudaFree(c->d_offsets);
     cudaFree(c->d_counters);
+    cudaFree(c->d_progress);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     topk_free(c->topk);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
@@ -159,6 +165,20 @@ ExpRec make_record(const dt_context *c, double t, const double *obs, double ra0,
     r.var = var;
     r.inv_var = 1.0 / var;
     return r;
+}
+
+// Lock-step window of kernel 3: the planes of window + 1 consecutive exposures (flux, and variance
+// in plane mode) should stay L2-resident while every orbit of the unit reads them.  Half of the L2
+// is budgeted (data read by SMs of both dies may be held once per die).  DT_GATHER_WINDOW overrides.
+int32_t pick_gather_window(const dt_context *c)
+{
+    const char *env = getenv("DT_GATHER_WINDOW");
+    if (env && atoi(env) > 0) return std::min(atoi(env), 64);
+    int l2 = 0;
+    if (cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, c->device) != cudaSuccess || l2 <= 0) l2 = 64 << 20;
+    const int64_t per_exp = c->plane * 4 * (c->var_mode == 1 ? 2 : 1);
+    int64_t w = ((int64_t)l2 / 2) / std::max<int64_t>(per_exp, 1) - 1;
+    return (int32_t)std::max<int64_t>(1, std::min<int64_t>(w, 16));
 }
 
 int mem_kind_ok(int32_t k) { return k == DT_MEM_HOST || k == DT_MEM_PINNED || k == DT_MEM_DEVICE; }
@@ -254,6 +274,10 @@ int dt_create(const dt_survey *s, dt_context **out)
         if (cudaMemcpyAsync(c->d_exp, c->h_exp.data(), sizeof(ExpRec) * (size_t)c->N, cudaMemcpyHostToDevice,
                             c->stream) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
         if (cudaMalloc((void **)&c->d_counters, 8 * sizeof(unsigned long long)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
+        if (cudaMalloc((void **)&c->d_progress, (size_t)(kMaxUnitExposures + kGroup) * sizeof(int)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
+        c->gather_window = pick_gather_window(c);
+        if (const char *env = getenv("DT_GATHER_L1")) c->gather_ld_cached = atoi(env) ? 1 : 0;
+        if (const char *env = getenv("DT_GATHER_LOCKSTEP")) c->gather_lockstep = atoi(env) < 0 ? -1 : (atoi(env) ? 1 : 0);
         if (cudaStreamSynchronize(c->stream) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
         size_t free_b = 0, total_b = 0;
         if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
@@ -495,8 +519,13 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
             g.S = c->d_S + o0;
             g.Wt = c->d_Wt + o0;
             g.cnt = c->d_cnt + o0;
-            CU(c, launch_gather(g, c->stream));
-            st.gather_launches += 1;
+            g.progress = c->d_progress;
+            g.window = c->gather_window;
+            g.n_hits_dev = c->d_counters;            // the unit's hit allocator, final after kernel 1
+            g.lockstep_mode = c->gather_lockstep;
+            g.ld_cached = c->gather_ld_cached;
+            CU(c, launch_gather(g, c->device, c->stream));
+            st.gather_launches += (c->gather_lockstep < 0) ? 2 : 1;   // sparse + dense schedule, one of them returns at once
             CU(c, cudaEventRecord(ev_at(3 * unit_idx + 2), c->stream));
             unit_idx += 1;
         }
@@ -609,12 +638,15 @@ int dt_project(dt_context *c, const double *elements, int64_t n, double t0, doub
 }
 
 int dt_gather_hits(dt_context *c, int64_t n, int32_t first_exposure, int32_t n_groups, const uint32_t *mask,
-                   const uint64_t *base, const uint32_t *offsets, double *S, double *Wt, int32_t *cnt)
+                   const uint64_t *base, const uint32_t *offsets, int64_t n_hits, double *S, double *Wt, int32_t *cnt)
 {
     if (!c) return DT_ERR_INVALID_ARG;
-    if (n < 0 || n_groups < 0 || first_exposure < 0 || (int64_t)first_exposure + (int64_t)n_groups * kGroup > (c->N + kGroup - 1) / kGroup * kGroup ||
+    if (n < 0 || n_hits < 0 || n_hits >= ((int64_t)1 << 32) || n_groups < 0 || first_exposure < 0 || (int64_t)first_exposure + (int64_t)n_groups * kGroup > (c->N + kGroup - 1) / kGroup * kGroup ||
         !mask || !base || !offsets || !S || !Wt || !cnt)
         return fail(c, DT_ERR_INVALID_ARG, "dt_gather_hits: bad arguments");
+    if (n > kMaxUnitOrbits || n_groups > kMaxUnitExposures / kGroup)
+        return fail(c, DT_ERR_INVALID_ARG, "dt_gather_hits: at most %lld orbits and %d groups per call",
+                    (long long)kMaxUnitOrbits, kMaxUnitExposures / kGroup);
     if (c->streaming || !c->d_flux) return fail(c, DT_ERR_STATE, "dt_gather_hits needs resident images");
     CU(c, cudaSetDevice(c->device));
     GatherParams g;
@@ -633,7 +665,13 @@ int dt_gather_hits(dt_context *c, int64_t n, int32_t first_exposure, int32_t n_g
     g.S = S;
     g.Wt = Wt;
     g.cnt = cnt;
-    CU(c, launch_gather(g, c->stream));
+    g.progress = c->d_progress;
+    g.window = c->gather_window;
+    g.n_hits_dev = nullptr;
+    g.n_hits_host = n_hits;
+    g.lockstep_mode = c->gather_lockstep;
+    g.ld_cached = c->gather_ld_cached;
+    CU(c, launch_gather(g, c->device, c->stream));
     return DT_OK;
 }
 

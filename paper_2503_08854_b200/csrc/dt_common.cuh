@@ -40,7 +40,7 @@ struct PropagateParams {
     double cx, cy, W, H;        // (W-1)/2, (H-1)/2, width, height as fp64
     int32_t width;
     double tan_fov;             // tan of the footprint half-diagonal, for the conservative pre-cull
-    // outputs of the cull + compaction stage (orbit-major hit list, see dtrack.h dt_gather_hits)
+    // outputs of the cull + compaction stage (hit list format: dtrack.h dt_gather_hits)
     uint32_t *mask;             // [n_groups][n_pad]
     unsigned long long *base;   // [n_groups][n_pad/32]
     uint32_t *offsets;          // [capacity]
@@ -68,9 +68,19 @@ struct GatherParams {
     int64_t plane;              // pixels per plane
     double *S, *Wt;             // [n] running sums (read-modify-write once per launch)
     int32_t *cnt;               // [n]
+    int *progress;              // [n_groups * 32] per-exposure count of CTAs that are done with it
+    int32_t window;             // lock-step window: exposure j starts after j - window is finished
+    int32_t tiles_per_warp;     // filled in by launch_gather
+    const unsigned long long *n_hits_dev;   // hits of the unit on the device (kernel 1's counter) or NULL
+    int64_t n_hits_host;        // used when n_hits_dev is NULL
+    int32_t lockstep_mode;      // -1: decide from the hit density; 0: sparse schedule; 1: dense schedule
+    int32_t ld_cached;          // dense schedule: pixel loads allocate in L1 (1) or not (0)
 };
 
-cudaError_t launch_gather(const GatherParams &p, cudaStream_t stream);
+constexpr int kGatherThreads = 512;     // 16 warps per CTA, two CTAs per SM
+constexpr int kMaxTilesPerWarp = 8;     // 148 SMs x 32 warps x 8 tiles x 32 orbits >= 2^20 orbits
+
+cudaError_t launch_gather(const GatherParams &p, int device, cudaStream_t stream);
 
 // SNR finalisation: snr = S / sqrt(Wt) (0 when no hit), NaN / -1 for invalid orbits.
 cudaError_t launch_finalize(const double *elements, int64_t n, const double *S, const double *Wt,

@@ -1,40 +1,41 @@
-// dt_gather.cu -- kernel 3: gather + stack, and the SNR finalisation.
+// dt_gather.cu -- kernel 3: gather + stack (sparse schedule, launcher) and the SNR finalisation.
 //
 // Hot-path steps 8-9 of DESIGN.md (Algorithm 1 `FindLocalSignal` + the per-orbit combination,
 // PAPER.md:171-172, 182 "jointly combining the signal from all intersections").  The paper pulls
 // pixels on the CPU from mmap'd SSD files; here the images are in HBM.
 //
-// Mapping: the hit list is orbit-major (dtrack.h, dt_gather_hits).  One orbit per lane; a warp owns
-// the same 32 orbits kernel 1's warp owned.  Per exposure group a lane reads its 32-bit hit mask
-// (one coalesced 128-B row per warp), a warp scan of popcounts locates its run of pixel offsets,
-// and it walks its own hits in ASCENDING exposure order accumulating S += f/v, Wt += 1/v in fp64
-// REGISTERS -- no atomics, no shared memory, and the same summation order as the definition, so S
-// and Wt are bit-identical to a sequential evaluation.  All warps sweep the groups in the same
-// order, which bins the image reads by exposure (L2 locality); loads are issued four hits at a time
-// to keep several sectors in flight per lane.
+// Two schedules share the hit-list format (dtrack.h, dt_gather_hits: per (warp-tile, group) block the
+// pixel offsets are exposure-major, then lane-ascending) and the per-orbit arithmetic; each launch
+// enqueues both kernels and each kernel returns at once unless the unit's hit density, read on the
+// device from kernel 1's counter, is in its regime (no host synchronisation between the kernels):
+//   * k_gather_sparse (this file): one orbit per lane, one warp-tile per warp, many CTAs.  Per block
+//     the warp transposes its 32 per-orbit masks into 32 per-exposure column masks (32 ballots) and
+//     scans their popcounts; entry (lane, jj) sits at block start + prefix[jj] + popc(column[jj] &
+//     lanes below).  Every lane then walks ITS OWN hits in ascending exposure order, four in
+//     flight, so all lanes stay busy however few exposures a block touches.  Bound: the rate of
+//     random DRAM accesses (no reuse to exploit when hits are sparse).
+//   * k_gather_dense (dt_gather_dense.cu): one persistent wave sweeping the exposures in lock-step so
+//     that the planes being gathered from stay L2-resident while every orbit of the unit reads them.
+// Both accumulate S += f/v, Wt += 1/v per orbit in ascending exposure order in a lane-private
+// accumulator (registers here, shared memory in the dense kernel) -- no atomics, and bit-identical
+// to a sequential evaluation of the definition.
 #include "dt_common.cuh"
+#include "dt_gather.cuh"
 
 namespace dt {
 
-constexpr int kGatherThreads = 256;
-
-__device__ __forceinline__ float ld_stream(const float *p)
-{
-    // read-only path, no L1 allocation: a pixel is used once per hit; reuse, if any, is in L2
-    float v;
-    asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(v) : "l"(p));
-    return v;
-}
+constexpr int kSparseThreads = 256;
 
 template <bool PLANE_VAR>
-__global__ void __launch_bounds__(kGatherThreads) k_gather_stack(const GatherParams p)
+__global__ void __launch_bounds__(kSparseThreads) k_gather_sparse(const GatherParams p)
 {
+    if (gather_is_dense(p)) return;
     const int lane = threadIdx.x & 31;
-    const int64_t orbit = (int64_t)blockIdx.x * kGatherThreads + threadIdx.x;
+    const int64_t orbit = (int64_t)blockIdx.x * kSparseThreads + threadIdx.x;
     if (orbit >= p.n_pad) return;   // n_pad is a multiple of 32: whole warps leave together
-    const bool in_range = orbit < p.n_orbits;
     const int64_t tile = orbit >> 5;
     const int64_t n_tiles = p.n_pad >> 5;
+    const unsigned lt = (1u << lane) - 1u;
 
     double S = 0.0, Wt = 0.0;
     int32_t cnt = 0;
@@ -42,58 +43,60 @@ __global__ void __launch_bounds__(kGatherThreads) k_gather_stack(const GatherPar
 
     for (int g = 0; g < p.n_groups; ++g) {
         uint32_t bits = p.mask[(int64_t)g * p.n_pad + orbit];
-        const unsigned any = __ballot_sync(0xffffffffu, bits != 0u);
-        if (!any) continue;
-        const int c = __popc(bits);
+        if (!__any_sync(0xffffffffu, bits != 0u)) continue;
+        // ---- column masks (lane jj holds exposure jj's) and the entry index of each column ----
+        uint32_t col = 0;
+#pragma unroll
+        for (int jj = 0; jj < 32; ++jj) {
+            const unsigned b = __ballot_sync(0xffffffffu, (bits >> jj) & 1u);
+            if (lane == jj) col = b;
+        }
+        const int c = __popc(col);
         int incl = c;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
             const int v = __shfl_up_sync(0xffffffffu, incl, d);
             if (lane >= d) incl += v;
         }
-        const unsigned long long b0 = p.base[(int64_t)g * n_tiles + tile];
-        const uint32_t *offs = p.offsets + b0 + (unsigned long long)(incl - c);
+        const uint32_t pre = (uint32_t)p.base[(int64_t)g * n_tiles + tile] + (uint32_t)(incl - c);
         const int64_t j0 = (int64_t)p.first_exposure + (int64_t)g * kGroup;
         if (bits && !touched) {
             // carry across exposure units: start from the partial sums of the earlier units so the
-            // additions happen in exactly ascending-exposure order (bit-identical to the definition)
+            // additions happen in exactly ascending-exposure order
             S = p.S[orbit];
             Wt = p.Wt[orbit];
             cnt = p.cnt[orbit];
             touched = true;
         }
-
-        int k = 0;
-        while (bits) {
-            // up to four hits in flight
+        while (__any_sync(0xffffffffu, bits != 0u)) {
             int jj[4];
-            uint32_t off[4];
+            uint32_t idx[4], off[4];
             float f[4], vv[4];
-            int m = 0;
+            bool have[4];
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                if (bits) {
-                    jj[q] = __ffs(bits) - 1;
-                    bits &= bits - 1;
-                    off[q] = offs[k + q];
-                    m = q + 1;
-                } else {
-                    jj[q] = 0;
-                    off[q] = 0;
-                }
+                have[q] = bits != 0u;
+                jj[q] = have[q] ? __ffs(bits) - 1 : 0;
+                bits &= bits - 1u;                       // 0 stays 0
+                const uint32_t cj = __shfl_sync(0xffffffffu, col, jj[q]);
+                const uint32_t pj = __shfl_sync(0xffffffffu, pre, jj[q]);
+                idx[q] = pj + __popc(cj & lt);
             }
 #pragma unroll
+            for (int q = 0; q < 4; ++q) off[q] = have[q] ? p.offsets[idx[q]] : 0u;
+#pragma unroll
             for (int q = 0; q < 4; ++q) {
-                if (q < m) {
+                f[q] = 0.f;
+                vv[q] = 1.f;
+                if (have[q]) {
                     const int64_t a = (j0 + jj[q]) * p.plane + off[q];
-                    f[q] = ld_stream(p.flux + a);
-                    if (PLANE_VAR) vv[q] = ld_stream(p.var + a);
+                    f[q] = ld_pixel_stream(p.flux + a);
+                    if (PLANE_VAR) vv[q] = ld_pixel_stream(p.var + a);
                 }
             }
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                if (q < m) {
-                    const double fd = (double)f[q];
+                if (have[q]) {
                     double v, w;
                     if (PLANE_VAR) {
                         v = (double)vv[q];
@@ -103,32 +106,34 @@ __global__ void __launch_bounds__(kGatherThreads) k_gather_stack(const GatherPar
                         v = x.var;
                         w = x.inv_var;
                     }
-                    if (isfinite(fd) && isfinite(v) && v > 0.0) {
-                        S += fd / v;
-                        Wt += w;
-                        cnt += 1;
-                    }
+                    stack_one((double)f[q], v, w, S, Wt, cnt);
                 }
             }
-            k += m;
         }
     }
-    if (in_range && touched) {
+    if (touched && orbit < p.n_orbits) {
         p.S[orbit] = S;
         p.Wt[orbit] = Wt;
         p.cnt[orbit] = cnt;
     }
 }
 
-cudaError_t launch_gather(const GatherParams &p, cudaStream_t stream)
+cudaError_t launch_gather(const GatherParams &p_in, int device, cudaStream_t stream)
 {
-    if (p.n_orbits <= 0 || p.n_groups <= 0) return cudaSuccess;
-    const unsigned blocks = (unsigned)((p.n_pad + kGatherThreads - 1) / kGatherThreads);
-    if (p.var)
-        k_gather_stack<true><<<blocks, kGatherThreads, 0, stream>>>(p);
-    else
-        k_gather_stack<false><<<blocks, kGatherThreads, 0, stream>>>(p);
-    return cudaGetLastError();
+    if (p_in.n_orbits <= 0 || p_in.n_groups <= 0) return cudaSuccess;
+    GatherParams p = p_in;
+    if (p.window < 1) p.window = 1;
+    if (p.lockstep_mode != 1) {
+        const unsigned blocks = (unsigned)((p.n_pad + kSparseThreads - 1) / kSparseThreads);
+        if (p.var)
+            k_gather_sparse<true><<<blocks, kSparseThreads, 0, stream>>>(p);
+        else
+            k_gather_sparse<false><<<blocks, kSparseThreads, 0, stream>>>(p);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    if (p.lockstep_mode != 0) return launch_gather_dense(p, device, stream);
+    return cudaSuccess;
 }
 
 // ---- finalisation ---------------------------------------------------------------------------------------

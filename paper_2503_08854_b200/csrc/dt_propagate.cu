@@ -9,10 +9,11 @@
 // exposures in time order carrying its Kepler state, so consecutive solves are warm-started.
 // Exposure records (128 B each) are staged group by group (32 exposures = 4 KB) into shared memory
 // by 1-D TMA bulk copies (cp.async.bulk, SASS UBLKCP) on a two-slot mbarrier ring; every lane
-// reads the same record (broadcast).  Hits are compacted per warp and group: each lane stages its
-// pixel offsets in shared memory, a warp scan turns the per-lane counts into an orbit-major
-// layout, one lane reserves the range with a single integer atomicAdd, and the 32 hit masks of
-// the group are written as one coalesced 128-B row.
+// reads the same record (broadcast).  Hits are compacted per warp and group with warp ballots:
+// at every exposure the hitting lanes append their pixel offsets, in lane order, to the warp's
+// shared-memory stage (so the stage is exposure-major, then lane-ascending); at the end of the
+// group one lane reserves the range with a single integer atomicAdd, the warp copies the stage
+// out with coalesced stores, and the 32 per-orbit hit masks are written as one coalesced 128-B row.
 #include "dt_common.cuh"
 #include "dt_orbit.cuh"
 
@@ -59,7 +60,7 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 
 struct __align__(128) PropSmem {
     ExpRec rec[2][kGroup];                       // 8 KB: two-slot ring of exposure groups
-    uint32_t stage[kWarpsPerCta][kGroup][32];    // 32 KB: [warp][slot][lane] staged pixel offsets
+    uint32_t stage[kWarpsPerCta][kGroup * 32];   // 32 KB: [warp][hit] staged pixel offsets
     uint64_t full[2];
 };
 
@@ -121,7 +122,8 @@ __global__ void __launch_bounds__(kTileOrbits, 2) k_propagate(const PropagatePar
         if (WARM && have_state) K = kepler_refresh(o.e, K);
 
         uint32_t bits = 0;
-        int cnt = 0;
+        int cnt = 0;          // this lane's hits in the group
+        int run = 0;          // the warp's hits in the group so far (warp-uniform)
         for (int jj = 0; jj < nrec; ++jj) {
             const ExpRec &x = sm.rec[slot][jj];
             const double dt = x.t - p.t0;
@@ -213,30 +215,31 @@ __global__ void __launch_bounds__(kTileOrbits, 2) k_propagate(const PropagatePar
                         p.pix[k + 1] = iy;
                     }
                 }
-            } else if (hit) {
-                sm.stage[warp][cnt][lane] = (uint32_t)iy * (uint32_t)p.width + (uint32_t)ix;
-                bits |= 1u << jj;
-                cnt += 1;
+            } else {
+                // ---- cull + compaction, stage 1: ballot-compact this exposure's hits ----
+                const unsigned hm = __ballot_sync(0xffffffffu, hit);
+                if (hm) {
+                    if (hit) {
+                        sm.stage[warp][run + __popc(hm & ((1u << lane) - 1u))] =
+                            (uint32_t)iy * (uint32_t)p.width + (uint32_t)ix;
+                        bits |= 1u << jj;
+                        cnt += 1;
+                    }
+                    run += __popc(hm);
+                }
             }
         }
 
         n_hits += (unsigned long long)cnt;
         if (!DENSE) {
-            // ---- warp-level compaction of the group's hits (orbit-major) ----
-            const unsigned any = __ballot_sync(0xffffffffu, cnt > 0);
-            int incl = cnt;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const int v = __shfl_up_sync(0xffffffffu, incl, d);
-                if (lane >= d) incl += v;
-            }
-            const int total = __shfl_sync(0xffffffffu, incl, 31);
+            // ---- stage 2: reserve the range, copy the stage out (exposure-major, coalesced) ----
             unsigned long long b0 = 0;
-            if (any) {
-                if (lane == 0) b0 = atomicAdd(p.counters, (unsigned long long)total);
+            if (run) {
+                if (lane == 0) b0 = atomicAdd(p.counters, (unsigned long long)run);
                 b0 = __shfl_sync(0xffffffffu, b0, 0);
-                uint32_t *dst = p.offsets + b0 + (unsigned long long)(incl - cnt);
-                for (int k = 0; k < cnt; ++k) dst[k] = sm.stage[warp][k][lane];
+                __syncwarp();
+                uint32_t *dst = p.offsets + b0;
+                for (int k = lane; k < run; k += 32) dst[k] = sm.stage[warp][k];
             }
             const int64_t opad = (int64_t)blockIdx.x * kTileOrbits + tid;
             if (opad < p.n_pad) {

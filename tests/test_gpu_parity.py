@@ -294,7 +294,7 @@ def test_more_than_one_orbit_unit():
 
 
 def test_gather_hits_entry_matches_definition():
-    """dt_gather_hits on a hand-built orbit-major hit list: every pair hits a seeded random pixel."""
+    """dt_gather_hits on a hand-built hit list: every pair hits a seeded random pixel."""
     dt = _dt()
     N, H, W, n = 64, 96, 80, 1000
     rng = np.random.default_rng(5)
@@ -312,8 +312,8 @@ def test_gather_hits_entry_matches_definition():
     for g in range(G):
         for w in range(npad // 32):
             base[g, w] = len(offsets)
-            for o in range(32 * w, 32 * w + 32):
-                for b in range(32):
+            for b in range(32):                       # exposure-ascending, then lane-ascending
+                for o in range(32 * w, 32 * w + 32):
                     if hit[32 * g + b, o]:
                         mask[g, o] |= np.uint32(1 << b)
                         offsets.append(pixel[32 * g + b, o])
@@ -333,7 +333,7 @@ def test_gather_hits_entry_matches_definition():
         dc = torch.zeros(n, dtype=torch.int32, device="cuda")
         trk.gather_hits(n, 0, G, torch.from_numpy(mask.view(np.int32)).cuda(),
                         torch.from_numpy(base.view(np.int64)).cuda(),
-                        torch.from_numpy(offsets.view(np.int32)).cuda(), dS, dW, dc)
+                        torch.from_numpy(offsets.view(np.int32)).cuda(), len(offsets), dS, dW, dc)
         torch.cuda.synchronize()
     assert np.array_equal(dc.cpu().numpy(), hit[:, :n].sum(0).astype(np.int32))
     assert np.array_equal(dS.cpu().numpy(), S) and np.array_equal(dW.cpu().numpy(), Wt)
