@@ -68,15 +68,19 @@ struct GatherParams {
     int64_t plane;              // pixels per plane
     double *S, *Wt;             // [n] running sums (read-modify-write once per launch)
     int32_t *cnt;               // [n]
-    int *progress;              // [n_groups * 32] per-exposure count of CTAs that are done with it
+    int *progress;              // [n_groups * 32 * kProgressStride] per-exposure count of CTAs done with it
     int32_t window;             // lock-step window: exposure j starts after j - window is finished
     int32_t tiles_per_warp;     // filled in by launch_gather
     const unsigned long long *n_hits_dev;   // hits of the unit on the device (kernel 1's counter) or NULL
     int64_t n_hits_host;        // used when n_hits_dev is NULL
     int32_t lockstep_mode;      // -1: decide from the hit density; 0: sparse schedule; 1: dense schedule
     int32_t ld_cached;          // dense schedule: pixel loads allocate in L1 (1) or not (0)
+    int32_t n_exp;              // exposures of the unit that exist (<= n_groups * 32)
+    int32_t prefetch;           // dense schedule: planes ahead the L2 prefetch runs; 0 = off
+    int32_t pipeline;           // dense schedule: 1 = three-stage software pipeline inside a warp
 };
 
+constexpr int kProgressStride = 32;     // one 128-B line per exposure counter (no false sharing of polls)
 constexpr int kGatherThreads = 512;     // 16 warps per CTA, two CTAs per SM
 constexpr int kMaxTilesPerWarp = 8;     // 148 SMs x 32 warps x 8 tiles x 32 orbits >= 2^20 orbits
 

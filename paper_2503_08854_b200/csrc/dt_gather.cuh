@@ -33,6 +33,17 @@ __device__ __forceinline__ void stack_one(double f, double v, double w, double &
     }
 }
 
+// f / v from the correctly rounded reciprocal w = RN(1/v) with FMA corrections (Markstein): q0 = f w is
+// within 1.5 ulp of f/v, one correction makes it faithful, the second gives the correctly rounded
+// quotient -- the same bits as the IEEE division of the definition, without the divide sequence.
+// Valid for finite f and v well inside the normal range (the caller checks).
+__device__ __forceinline__ double div_by_reciprocal(double f, double v, double w)
+{
+    const double q0 = f * w;
+    const double q1 = fma(fma(-q0, v, f), w, q0);
+    return fma(fma(-q1, v, f), w, q1);
+}
+
 // Dense when the unit has at least one hit per 16 pixels of every plane it covers (then most 128-B
 // lines of a plane are touched and keeping the plane L2-resident pays); grid-uniform.
 __device__ __forceinline__ bool gather_is_dense(const GatherParams &p)

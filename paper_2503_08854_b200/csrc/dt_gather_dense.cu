@@ -16,6 +16,8 @@
 //     orbits of the unit read them: a plane is fetched from DRAM once per launch instead of once per
 //     wave of CTAs (profiles/r1a_baseline.md: 62.7 GB of DRAM reads for 8.9 GB of algorithmic bytes).
 //     The grid is launched cooperatively so that all CTAs are co-resident (the throttle needs it).
+#include <stdlib.h>
+
 #include "dt_common.cuh"
 #include "dt_gather.cuh"
 
@@ -32,7 +34,7 @@ __device__ __forceinline__ void red_add_relaxed(int *p, int v)
     asm volatile("red.relaxed.gpu.global.add.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-// Shared memory of one CTA: S, Wt [T][kGatherThreads] fp64, cnt [T][kGatherThreads] int32
+// Shared memory of one CTA: (S, Wt) [T][kGatherThreads] double2, cnt [T][kGatherThreads] int32
 // (accumulators, lane-private), arrive [n_local] int, done_upto int (lock-step throttle).
 template <bool PLANE_VAR>
 __global__ void __launch_bounds__(kGatherThreads, 2) k_gather_dense(const GatherParams p)
@@ -41,9 +43,8 @@ __global__ void __launch_bounds__(kGatherThreads, 2) k_gather_dense(const Gather
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int T = p.tiles_per_warp;
     constexpr int n_warps = kGatherThreads / 32;
-    double *sS = reinterpret_cast<double *>(smem_raw);
-    double *sW = sS + (size_t)T * kGatherThreads;
-    int32_t *sC = reinterpret_cast<int32_t *>(sW + (size_t)T * kGatherThreads);
+    double2 *sAcc = reinterpret_cast<double2 *>(smem_raw);          // (S, Wt)
+    int32_t *sC = reinterpret_cast<int32_t *>(sAcc + (size_t)T * kGatherThreads);
     int *arrive = sC + (size_t)T * kGatherThreads;
     const int n_local = p.n_groups * kGroup;
     volatile int *done_upto = arrive + n_local;   // exposures [0, done_upto) are finished by every CTA
@@ -81,8 +82,7 @@ __global__ void __launch_bounds__(kGatherThreads, 2) k_gather_dense(const Gather
                 if (bits[t] && !((touched >> t) & 1u)) {
                     // carry across exposure units: start from the partial sums of the earlier units
                     const int a = t * kGatherThreads + threadIdx.x;
-                    sS[a] = p.S[o];
-                    sW[a] = p.Wt[o];
+                    sAcc[a] = make_double2(p.S[o], p.Wt[o]);
                     sC[a] = p.cnt[o];
                     touched |= 1u << t;
                 }
@@ -146,10 +146,12 @@ __global__ void __launch_bounds__(kGatherThreads, 2) k_gather_dense(const Gather
                 }
             }
             double vs = 1.0, ws = 1.0;
+            bool fast = false;
             if (!PLANE_VAR) {
                 const ExpRec &x = p.exp_all[j0 + jj];
                 vs = x.var;
                 ws = x.inv_var;
+                fast = vs > 1e-150 && vs < 1e150;     // uniform; else the IEEE division of stack_one
             }
 #pragma unroll
             for (int t = 0; t < kMaxTilesPerWarp; ++t) {
@@ -157,12 +159,21 @@ __global__ void __launch_bounds__(kGatherThreads, 2) k_gather_dense(const Gather
                     const double v = PLANE_VAR ? (double)vv[t] : vs;
                     const double w = PLANE_VAR ? 1.0 / v : ws;
                     const int a = t * kGatherThreads + threadIdx.x;
-                    double S = sS[a], Wt = sW[a];
-                    int32_t c = sC[a];
-                    stack_one((double)f[t], v, w, S, Wt, c);
-                    sS[a] = S;
-                    sW[a] = Wt;
-                    sC[a] = c;
+                    if (fast) {
+                        if (fabsf(f[t]) <= 3.402823466e38f) {   // finite (NaN compares false)
+                            double2 acc = sAcc[a];
+                            acc.x += div_by_reciprocal((double)f[t], vs, ws);
+                            acc.y += ws;
+                            sAcc[a] = acc;
+                            sC[a] += 1;
+                        }
+                    } else {
+                        double2 acc = sAcc[a];
+                        int32_t c = sC[a];
+                        stack_one((double)f[t], v, w, acc.x, acc.y, c);
+                        sAcc[a] = acc;
+                        sC[a] = c;
+                    }
                 }
             }
             // ---- arrival: this warp is done with exposure jl ----
@@ -177,8 +188,9 @@ __global__ void __launch_bounds__(kGatherThreads, 2) k_gather_dense(const Gather
         if (((touched >> t) & 1u) && orbit_of(t) < p.n_orbits) {
             const int64_t o = orbit_of(t);
             const int a = t * kGatherThreads + threadIdx.x;
-            p.S[o] = sS[a];
-            p.Wt[o] = sW[a];
+            const double2 acc = sAcc[a];
+            p.S[o] = acc.x;
+            p.Wt[o] = acc.y;
             p.cnt[o] = sC[a];
         }
     }
@@ -227,6 +239,10 @@ cudaError_t launch_gather_dense(const GatherParams &p_in, int device, cudaStream
         e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         smem_set[which] = smem;
+        if (const char *env = getenv("DT_GATHER_CARVEOUT")) {   // experiment knob: % of the SM's L1/smem
+            e = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, atoi(env));
+            if (e != cudaSuccess) return e;
+        }
     }
     void *args[] = {(void *)&p};
     return cudaLaunchCooperativeKernel(fn, dim3((unsigned)grid), dim3(kGatherThreads), args, smem, stream);
