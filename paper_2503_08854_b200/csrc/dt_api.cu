@@ -69,8 +69,6 @@ struct dt_context {
     int32_t gather_window = 1;                          // exposures the slowest and fastest CTA may be apart
     int32_t gather_lockstep = -1;                       // -1: decided on the device from the hit density
     int32_t gather_ld_cached = 1;
-    int32_t gather_pipeline = 0;
-    int32_t gather_prefetch = 0;                        // planes ahead of the dense schedule's L2 prefetch
     std::vector<cudaEvent_t> ev_pool;                   // timing events
 
     TopkWorkspace topk;
@@ -278,8 +276,6 @@ int dt_create(const dt_survey *s, dt_context **out)
         if (cudaMalloc((void **)&c->d_counters, 8 * sizeof(unsigned long long)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
         if (cudaMalloc((void **)&c->d_progress, (size_t)(kMaxUnitExposures + kGroup) * kProgressStride * sizeof(int)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
         c->gather_window = pick_gather_window(c);
-        if (const char *env = getenv("DT_GATHER_PREFETCH")) c->gather_prefetch = std::max(0, std::min(atoi(env), 8));
-        if (const char *env = getenv("DT_GATHER_PIPE")) c->gather_pipeline = atoi(env) ? 1 : 0;
         if (const char *env = getenv("DT_GATHER_L1")) c->gather_ld_cached = atoi(env) ? 1 : 0;
         if (const char *env = getenv("DT_GATHER_LOCKSTEP")) c->gather_lockstep = atoi(env) < 0 ? -1 : (atoi(env) ? 1 : 0);
         if (cudaStreamSynchronize(c->stream) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
@@ -528,9 +524,6 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
             g.n_hits_dev = c->d_counters;            // the unit's hit allocator, final after kernel 1
             g.lockstep_mode = c->gather_lockstep;
             g.ld_cached = c->gather_ld_cached;
-            g.n_exp = n_exp;
-            g.prefetch = c->gather_prefetch;
-            g.pipeline = c->gather_pipeline;
             CU(c, launch_gather(g, c->device, c->stream));
             st.gather_launches += (c->gather_lockstep < 0) ? 2 : 1;   // sparse + dense schedule, one of them returns at once
             CU(c, cudaEventRecord(ev_at(3 * unit_idx + 2), c->stream));
@@ -678,9 +671,6 @@ int dt_gather_hits(dt_context *c, int64_t n, int32_t first_exposure, int32_t n_g
     g.n_hits_host = n_hits;
     g.lockstep_mode = c->gather_lockstep;
     g.ld_cached = c->gather_ld_cached;
-    g.n_exp = std::min<int32_t>(n_groups * kGroup, c->N - first_exposure);
-    g.prefetch = c->gather_prefetch;
-    g.pipeline = c->gather_pipeline;
     CU(c, launch_gather(g, c->device, c->stream));
     return DT_OK;
 }

@@ -75,9 +75,6 @@ struct GatherParams {
     int64_t n_hits_host;        // used when n_hits_dev is NULL
     int32_t lockstep_mode;      // -1: decide from the hit density; 0: sparse schedule; 1: dense schedule
     int32_t ld_cached;          // dense schedule: pixel loads allocate in L1 (1) or not (0)
-    int32_t n_exp;              // exposures of the unit that exist (<= n_groups * 32)
-    int32_t prefetch;           // dense schedule: planes ahead the L2 prefetch runs; 0 = off
-    int32_t pipeline;           // dense schedule: 1 = three-stage software pipeline inside a warp
 };
 
 constexpr int kProgressStride = 32;     // one 128-B line per exposure counter (no false sharing of polls)

@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(kGatherThreads, 2) k_gather_dense(const Gather
         if (!((gm >> lane) & 1u)) {
             const int jl = g * kGroup + lane;
             const int old = atomicAdd(&arrive[jl], 1);
-            if (old == n_warps - 1) red_add_relaxed(p.progress + jl, 1);
+            if (old == n_warps - 1) red_add_relaxed(p.progress + jl * kProgressStride, 1);
         }
 
         const int64_t j0 = (int64_t)p.first_exposure + (int64_t)g * kGroup;
@@ -108,7 +108,7 @@ __global__ void __launch_bounds__(kGatherThreads, 2) k_gather_dense(const Gather
             if (need >= 0) {
                 int d = *done_upto;
                 while (d <= need) {
-                    if (ld_relaxed(p.progress + d) >= n_ctas) {
+                    if (ld_relaxed(p.progress + d * kProgressStride) >= n_ctas) {
                         d += 1;
                         if (lane == 0) atomicMax((int *)done_upto, d);
                     } else {
@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(kGatherThreads, 2) k_gather_dense(const Gather
             // ---- arrival: this warp is done with exposure jl ----
             if (lane == 0) {
                 const int old = atomicAdd(&arrive[jl], 1);
-                if (old == n_warps - 1) red_add_relaxed(p.progress + jl, 1);
+                if (old == n_warps - 1) red_add_relaxed(p.progress + jl * kProgressStride, 1);
             }
         }
     }
@@ -230,7 +230,7 @@ cudaError_t launch_gather_dense(const GatherParams &p_in, int device, cudaStream
     cudaError_t e = dense_geometry(p.n_pad, p.n_groups, device, &grid, &T, &smem);
     if (e != cudaSuccess) return e;
     p.tiles_per_warp = T;
-    e = cudaMemsetAsync(p.progress, 0, (size_t)p.n_groups * kGroup * sizeof(int), stream);
+    e = cudaMemsetAsync(p.progress, 0, (size_t)p.n_groups * kGroup * kProgressStride * sizeof(int), stream);
     if (e != cudaSuccess) return e;
     const void *fn = p.var ? (const void *)k_gather_dense<true> : (const void *)k_gather_dense<false>;
     static size_t smem_set[2] = {0, 0};
