@@ -39,7 +39,7 @@ FP64_SLOTS_REFINE = 84.0     # light-time re-solve + projection + footprint test
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="small_mba")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
