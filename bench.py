@@ -378,7 +378,7 @@ def main():
                 "roofline": roofline,
                 "stages_ms": {"propagate": float(np.mean(ms_prop)), "gather": float(np.mean(ms_gath)),
                               "finalize": stats["ms_finalize"]},
-                "hits_per_step": int(stats["hits"]), "cold_solves": int(stats["cold_solves"]),
+                "hits_per_step": int(stats["hits"]), "cold_solves": int(stats["cold_solves"]), "substep_solves": int(stats["substep_solves"]),
                 "wall_s_timed_region": wall}
         if not args.no_gather_bench:
             hbm, src = measured_hbm_peak()

@@ -99,6 +99,7 @@ typedef struct {
     int64_t invalid_orbits;    /* orbits rejected (a <= 0, e outside [0,1), non-finite)           */
     int64_t refined_pairs;     /* pairs that went through light-time refinement + projection      */
     int64_t cold_solves;       /* Kepler solves started cold (libdevice sincos Newton)            */
+    int64_t substep_solves;    /* Kepler solves advanced by several warm sub-steps                */
     int64_t h2d_image_bytes;   /* image bytes streamed host -> device inside the call             */
     int32_t streamed;          /* 1 when the image store did not fit and batches were streamed    */
     int32_t n_image_batches;   /* exposure ranges processed                                       */

@@ -51,7 +51,7 @@ class dt_stats(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("n_orbits", C.c_int64), ("n_exposures", C.c_int64),
                 ("pairs", C.c_int64), ("hits", C.c_int64), ("invalid_orbits", C.c_int64),
                 ("refined_pairs", C.c_int64), ("cold_solves", C.c_int64),
-                ("h2d_image_bytes", C.c_int64), ("streamed", C.c_int32), ("n_image_batches", C.c_int32),
+                ("substep_solves", C.c_int64), ("h2d_image_bytes", C.c_int64), ("streamed", C.c_int32), ("n_image_batches", C.c_int32),
                 ("ms_total", C.c_float), ("ms_propagate", C.c_float), ("ms_gather", C.c_float),
                 ("ms_finalize", C.c_float), ("launches", C.c_int32), ("propagate_launches", C.c_int32),
                 ("gather_launches", C.c_int32)]

@@ -558,6 +558,7 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
     st.hits = (int64_t)hc[3];
     st.refined_pairs = (int64_t)hc[1];
     st.cold_solves = (int64_t)hc[2];
+    st.substep_solves = (int64_t)hc[4];
     st.invalid_orbits = (int64_t)hc[5];
     st.launches = st.propagate_launches + st.gather_launches + 1;
     c->n_last = n;

@@ -36,6 +36,7 @@ __global__ void __launch_bounds__(kSparseThreads) k_gather_sparse(const GatherPa
     const int64_t tile = orbit >> 5;
     const int64_t n_tiles = p.n_pad >> 5;
     const unsigned lt = (1u << lane) - 1u;
+    const bool cached = p.ld_cached != 0;
 
     double S = 0.0, Wt = 0.0;
     int32_t cnt = 0;
@@ -90,8 +91,13 @@ __global__ void __launch_bounds__(kSparseThreads) k_gather_sparse(const GatherPa
                 vv[q] = 1.f;
                 if (have[q]) {
                     const int64_t a = (j0 + jj[q]) * p.plane + off[q];
-                    f[q] = ld_pixel_stream(p.flux + a);
-                    if (PLANE_VAR) vv[q] = ld_pixel_stream(p.var + a);
+                    if (cached) {
+                        f[q] = ld_pixel_cached(p.flux + a);
+                        if (PLANE_VAR) vv[q] = ld_pixel_cached(p.var + a);
+                    } else {
+                        f[q] = ld_pixel_stream(p.flux + a);
+                        if (PLANE_VAR) vv[q] = ld_pixel_stream(p.var + a);
+                    }
                 }
             }
 #pragma unroll

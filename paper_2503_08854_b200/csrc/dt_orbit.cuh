@@ -222,6 +222,20 @@ __device__ __forceinline__ Kepler kepler_warm(double e, const Kepler &K0, double
     return K;
 }
 
+// How far outside kepler_warm's accuracy domain a step toward Mn is: the step is acceptable when the
+// returned ratio is <= 1 (same two tests as `ok` there); a step with ratio r is split by the caller
+// into ceil(1.5 r) equal sub-steps in M, each a full warm step (series + rotation + Newton polish
+// against its own directly computed M), which stays far cheaper than a cold solve up to ~10 of them.
+__device__ __forceinline__ float kepler_warm_need(double e, const Kepler &K0, double Mn)
+{
+    const double dM = Mn - K0.M;
+    const double es = e * K0.s;
+    const double rg = rcp_nr<1>(fma(-e, K0.c, 1.0));
+    const double x = ((K0.u - es) - dM) * rg;
+    const double xa2 = x * (0.5 * es * rg);
+    return (float)fmax(fabs(x) * 25.0, fabs(xa2) * 100.0);
+}
+
 // Refresh: recompute (sin E, cos E) of the carried state exactly (libdevice sincos of the reduced
 // E = M + u) and polish u once, so the rounding of the Taylor rotations cannot accumulate beyond
 // one exposure group.

@@ -58,6 +58,8 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
         : "memory");
 }
 
+constexpr int kMaxSubsteps = 12;   // sub-steps of one warm Kepler step before the cold solve is cheaper
+
 struct __align__(128) PropSmem {
     ExpRec rec[2][kGroup];                       // 8 KB: two-slot ring of exposure groups
     uint32_t stage[kWarpsPerCta][kGroup * 32];   // 32 KB: [warp][hit] staged pixel offsets
@@ -111,7 +113,7 @@ __global__ void __launch_bounds__(kTileOrbits, 2) k_propagate(const PropagatePar
     K.M = K.u = K.s = 0.0;
     K.c = 1.0;
     bool have_state = false;
-    unsigned long long n_refined = 0, n_cold = 0, n_hits = 0;
+    unsigned long long n_refined = 0, n_cold = 0, n_hits = 0, n_sub = 0;
 
     for (int g = g_begin; g < g_end; ++g) {
         const int slot = (g - g_begin) & 1;
@@ -137,8 +139,34 @@ __global__ void __launch_bounds__(kTileOrbits, 2) k_propagate(const PropagatePar
                 if (__all_sync(0xffffffffu, ok)) {
                     K = Kw;
                 } else {
-                    K = kepler_cold(o.e, M);
-                    n_cold += 1;
+                    // some lane's step is too long for one warm step (long gap, or close to the
+                    // perihelion of an eccentric orbit): split it into equal sub-steps in M, the
+                    // count warp-uniform; only when that would take too many, solve cold
+                    bool solved = false;
+                    if (have_state) {
+                        const float r = __uint_as_float(
+                            __reduce_max_sync(0xffffffffu, __float_as_uint(kepler_warm_need(o.e, K, M))));
+                        if (r < (float)kMaxSubsteps / 1.5f) {       // false for NaN
+                            const int ns = max(2, (int)ceilf(1.5f * r));
+                            const double M_from = K.M, dMs = (M - M_from) / (double)ns;
+                            Kepler Kc = K;
+                            bool good = true;
+                            for (int sidx = 1; sidx <= ns; ++sidx) {
+                                bool oks;
+                                Kc = kepler_warm(o.e, Kc, (sidx == ns) ? M : fma(dMs, (double)sidx, M_from), oks);
+                                good = good && oks;
+                            }
+                            if (__all_sync(0xffffffffu, good)) {
+                                K = Kc;
+                                solved = true;
+                                n_sub += 1;
+                            }
+                        }
+                    }
+                    if (!solved) {
+                        K = kepler_cold(o.e, M);
+                        n_cold += 1;
+                    }
                 }
                 have_state = true;
             } else {
@@ -258,11 +286,13 @@ __global__ void __launch_bounds__(kTileOrbits, 2) k_propagate(const PropagatePar
         n_refined += __shfl_xor_sync(0xffffffffu, n_refined, d);
         n_cold += __shfl_xor_sync(0xffffffffu, n_cold, d);
         n_hits += __shfl_xor_sync(0xffffffffu, n_hits, d);
+        n_sub += __shfl_xor_sync(0xffffffffu, n_sub, d);
     }
     if (lane == 0 && p.counters) {
         atomicAdd(p.counters + 1, n_refined);
         atomicAdd(p.counters + 2, n_cold);
         if (n_hits) atomicAdd(p.counters + 3, n_hits);
+        if (n_sub) atomicAdd(p.counters + 4, n_sub);
     }
 }
 
