@@ -34,6 +34,9 @@ UNIT = "pairs/s"
 # counted from the SASS of k_propagate<3> and confirmed by ncu smsp__inst_executed_pipe_fp64):
 FP64_SLOTS_COARSE = 72.0     # warm Kepler step + geometric position + cone test (every pair)
 FP64_SLOTS_REFINE = 84.0     # light-time re-solve + projection + footprint test (refined pairs only)
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_propagate<3> launch on configs[1], from the
+# `ncu --set full` capture summarised in profiles/r1b_gather.md (48.52 MB + 19.53 MB)
+K1_TRAFFIC_BYTES_SMALL_MBA = 68.05e6
 
 
 def parse_args():
@@ -362,7 +365,10 @@ def main():
             slots = FP64_SLOTS_COARSE + FP64_SLOTS_REFINE
         achieved_tf = 2.0 * slots * pairs_per_launch / (ms_k1 * 1e-3) * 1e-12
         roofline = {"bound": "alu", "kernel": "k_propagate", "achieved": achieved_tf, "peak": peak_tf,
-                    "unit": "TFLOP/s", "frac": achieved_tf / peak_tf if peak_tf else None, "traffic": None,
+                    "unit": "TFLOP/s", "frac": achieved_tf / peak_tf if peak_tf else None,
+                    "traffic": K1_TRAFFIC_BYTES_SMALL_MBA if (cfg.name == "small_mba" and not args.orbits and
+                                                              not args.exposures and not args.flags) else None,
+                    "traffic_unit": "bytes per launch (ncu dram read + write, profiles/r1b_gather.md)",
                     "peak_source": "dt_fp64_peak DFMA probe measured in this run (MEASURED_PEAKS.json has no FP64 figure)",
                     "fp64_slots_per_pair": slots, "refined_fraction": refined_frac,
                     "ms_per_launch": ms_k1, "share_of_step": float(np.mean(ms_prop)) / ms_step}
