@@ -226,12 +226,28 @@ def gather_bench(dt, trk, cfg, dev, hbm_gbs, reps=5, regimes=None):
         bytes_min = (hl["hits"] * 4 + hl["mask"].numel() * 4 + hl["base"].numel() * 8 +
                      hl["unique_sectors"] * 32 * planes + hl["touched_orbits"] * 20)
         gbs = bytes_min / (ms * 1e-3) * 1e-9
+        # second bound: a fully divergent 4-B gather is served by the L1 at one lane per clock and SM
+        # (measured: the reuse regime, whose pixels hit L1, runs at 0.99 of it)
+        props = torch.cuda.get_device_properties(dev)
+        l1_rate = props.multi_processor_count * sm_clock_hz(dev.index or 0)
         out.append({"regime": name, "hits": hl["hits"], "unique_sectors": hl["unique_sectors"],
                     "bytes_min": int(bytes_min), "ms": ms, "hits_per_s": hl["hits"] / (ms * 1e-3),
-                    "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": gbs / hbm_gbs})
+                    "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": gbs / hbm_gbs,
+                    "l1_gather_bound": {"peak": l1_rate, "unit": "gathers/s",
+                                        "frac": hl["hits"] / (ms * 1e-3) / l1_rate}})
         del hl, S, Wt, cnt
         torch.cuda.empty_cache()
     return out
+
+
+def sm_clock_hz(index: int) -> float:
+    """Maximum SM clock (the benches run unthrottled at it; bench.py reports the sampled clocks too)."""
+    try:
+        out = subprocess.run(["nvidia-smi", "-i", str(index), "--query-gpu=clocks.max.sm",
+                              "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=10).stdout
+        return float(out.strip().splitlines()[0]) * 1e6
+    except Exception:
+        return 1.965e9
 
 
 def measured_hbm_peak():

@@ -58,6 +58,9 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
         : "memory");
 }
 
+#ifndef DT_K1_MIN_CTAS
+#define DT_K1_MIN_CTAS 2           // resident CTAs per SM kernel 1 is compiled for (register budget)
+#endif
 constexpr int kMaxSubsteps = 12;   // sub-steps of one warm Kepler step before the cold solve is cheaper
 
 struct __align__(128) PropSmem {
@@ -67,7 +70,7 @@ struct __align__(128) PropSmem {
 };
 
 template <int MODE>
-__global__ void __launch_bounds__(kTileOrbits, 2) k_propagate(const PropagateParams p)
+__global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const PropagateParams p)
 {
     constexpr bool WARM = (MODE & kModeWarm) != 0;
     constexpr bool PRECULL = (MODE & kModePrecull) != 0;
