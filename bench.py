@@ -258,6 +258,26 @@ def measured_hbm_peak():
         return 6650.0, "fallback 6.65 TB/s of B200_PROFILING.md (of fallback)"
 
 
+# ---- replicas (N > 1): the only cross-rank logic of the path --------------------------------------------
+def rank_elements(cfg, rank: int, world: int) -> np.ndarray:
+    """Rank r of N processes its own block of seeded candidates: indices [r n, (r+1) n) of the
+    config's orbit stream (weak scaling; no rank ever needs another rank's orbits or results)."""
+    n = cfg.n_orbits
+    return ds.elements(cfg, rank * n, (rank + 1) * n) if world > 1 else ds.elements(cfg, 0, n)
+
+
+def max_over_ranks(values, world: int, device=None):
+    """Element-wise MAX over ranks of a short list of timings (the only collective bench.py issues
+    besides the barriers)."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return [float(v) for v in tt]
+
+
 # ---- B200 arm ----------------------------------------------------------------------------------------------
 def main():
     args = parse_args()
@@ -290,7 +310,7 @@ def main():
 
     scene = ds.build_scene(cfg, project_fn)
     n = cfg.n_orbits
-    el_np = ds.elements(cfg, rank * n, (rank + 1) * n) if world > 1 else scene.elements()
+    el_np = rank_elements(cfg, rank, world)
     trk = dt.Tracker.from_scene(scene, device=local_rank, flags=args.flags)
     trk_holder["t"] = trk
     for j in range(cfg.n_exp):
@@ -342,15 +362,16 @@ def main():
     # ---- end to end: host (pinned) elements in, host results out, copies inside the timed region ----
     e2e = None
     if not args.no_e2e:
+        out_pin = (torch.empty(n, dtype=torch.float64).pin_memory(), torch.empty(n, dtype=torch.int32).pin_memory())
         for _ in range(2):
-            trk.stack(el_pin, scene.t0)
+            trk.stack(el_pin, scene.t0, out=out_pin)
         barrier()
         ms_e2e = []
         for _ in range(args.steps):
             flush.fill_(1)
             torch.cuda.synchronize()
             t0 = time.perf_counter()
-            snr_h, hits_h = trk.stack(el_pin, scene.t0)
+            snr_h, hits_h = trk.stack(el_pin, scene.t0, out=out_pin)
             ms_e2e.append((time.perf_counter() - t0) * 1e3)
         barrier()
         ms_e2e = float(np.mean(ms_e2e))
@@ -358,9 +379,7 @@ def main():
 
     # ---- max over ranks ----
     if world > 1:
-        tt = torch.tensor([ms_step, ms_e2e if not args.no_e2e else 0.0], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_step, ms_e2e_max = float(tt[0]), float(tt[1])
+        ms_step, ms_e2e_max = max_over_ranks([ms_step, ms_e2e if not args.no_e2e else 0.0], world, dev)
         if not args.no_e2e:
             ms_e2e = ms_e2e_max
     pairs_total = float(cfg.pairs) * world
@@ -368,7 +387,7 @@ def main():
     if not args.no_e2e:
         e2e = {"value": pairs_total / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(n * 48),
                "d2h_bytes_per_step": int(n * 12), "ms_per_step": ms_e2e,
-               "note": "dt_stack with pinned host elements and host outputs; images registered before"}
+               "note": "dt_stack with pinned host elements in, pinned host SNR/hits out; images registered before"}
 
     if rank == 0:
         # ---- roofline of the dominant kernel (kernel 1: FP64 ALU bound) ----

@@ -157,12 +157,27 @@ def dt_load_image_batch(ctx, first_exposure: int, flux, var=None) -> None:
     _check(lib().dt_load_image_batch(ctx, first_exposure, count, pf, pv, kind), ctx)
 
 
-def dt_stack(ctx, elements, t0: float):
+def dt_stack(ctx, elements, t0: float, out=None):
     """elements [n, 6] float64 (numpy or torch, host or CUDA) -> (snr [n] f64, hits [n] i32) in the
-    same kind of container."""
+    same kind of container.  `out` = (snr, hits) supplies the output buffers (same memory kind as the
+    elements: e.g. pinned torch tensors reused from call to call, so that the device->host copy does not
+    go through freshly allocated pageable memory)."""
     n = int(elements.shape[0])
     pe, kind = _ptr_kind(elements)
-    if _is_torch(elements):
+    if out is not None:
+        snr, hits = out
+        ps, kind_s = _ptr_kind(snr)
+        ph, kind_h = _ptr_kind(hits)
+        host = (DT_MEM_HOST, DT_MEM_PINNED)
+        if not (kind_s == kind_h == kind or (kind in host and kind_s in host and kind_h in host)):
+            raise ValueError("out buffers must live in the same kind of memory as the elements")
+        if int(snr.shape[0]) != n or int(hits.shape[0]) != n:
+            raise ValueError("out buffers must have n entries")
+        if str(snr.dtype).split(".")[-1] != "float64" or str(hits.dtype).split(".")[-1] != "int32":
+            raise ValueError("out = (float64 snr, int32 hits)")
+        if str(elements.dtype).split(".")[-1] != "float64":
+            raise ValueError("elements must be float64")
+    elif _is_torch(elements):
         import torch
         if elements.dtype != torch.float64:
             raise ValueError("elements must be float64")
@@ -238,8 +253,8 @@ class Tracker:
     def load_image_batch(self, first_exposure, flux, var=None):
         dt_load_image_batch(self.ctx, first_exposure, flux, var)
 
-    def stack(self, elements, t0=0.0):
-        return dt_stack(self.ctx, elements, t0)
+    def stack(self, elements, t0=0.0, out=None):
+        return dt_stack(self.ctx, elements, t0, out)
 
     def topk(self, k, min_hits=0):
         return dt_topk(self.ctx, k, min_hits)
