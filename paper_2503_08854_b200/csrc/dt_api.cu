@@ -6,6 +6,7 @@
 
 #include <math.h>
 #include <stdarg.h>
+#include <stdint.h>
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
@@ -69,6 +70,7 @@ struct dt_context {
     int32_t gather_window = 1;                          // exposures the slowest and fastest CTA may be apart
     int32_t gather_lockstep = -1;                       // -1: decided on the device from the hit density
     int32_t gather_ld_cached = 1;
+    bool zero_copy_elements = true;                     // DT_ZERO_COPY=0: copy pinned elements to the device first
     std::vector<cudaEvent_t> ev_pool;                   // timing events
 
     TopkWorkspace topk;
@@ -276,6 +278,7 @@ int dt_create(const dt_survey *s, dt_context **out)
         if (cudaMalloc((void **)&c->d_counters, 8 * sizeof(unsigned long long)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
         if (cudaMalloc((void **)&c->d_progress, (size_t)(kMaxUnitExposures + kGroup) * kProgressStride * sizeof(int)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
         c->gather_window = pick_gather_window(c);
+        if (const char *env = getenv("DT_ZERO_COPY")) c->zero_copy_elements = atoi(env) != 0;
         if (const char *env = getenv("DT_GATHER_L1")) c->gather_ld_cached = atoi(env) ? 1 : 0;
         if (const char *env = getenv("DT_GATHER_LOCKSTEP")) c->gather_lockstep = atoi(env) < 0 ? -1 : (atoi(env) ? 1 : 0);
         if (cudaStreamSynchronize(c->stream) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
@@ -401,11 +404,27 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
     const int32_t unit_exp = c->streaming ? c->batch_exp : std::min<int32_t>(c->N, kMaxUnitExposures);
     const int64_t unit_orb = std::min<int64_t>((n + 31) / 32 * 32, kMaxUnitOrbits);
     const int32_t unit_groups = (unit_exp + kGroup - 1) / kGroup;
-    const double *d_el = elements;
-    if (mem_kind != DT_MEM_DEVICE) {
+    // Elements: kernel 1 stages each tile with one bulk copy, from device memory or straight from
+    // page-locked host memory (first pass over the orbits; it leaves a device copy for later passes
+    // and for the finalisation).  Pageable or misaligned inputs are copied to the device first.
+    const double *d_el = elements;           // what later passes and k_finalize read
+    const double *first_src = elements;      // what the first pass of kernel 1 reads
+    double *copy_out = nullptr;
+    const bool aligned16 = (reinterpret_cast<uintptr_t>(elements) & 15u) == 0;
+    if (mem_kind != DT_MEM_DEVICE || !aligned16) {
         CU(c, grow(c->d_el, c->el_cap, n * 6));
-        CU(c, cudaMemcpyAsync(c->d_el, elements, (size_t)n * 48, cudaMemcpyHostToDevice, c->stream));
         d_el = c->d_el;
+        void *mapped = nullptr;
+        if (mem_kind == DT_MEM_PINNED && aligned16 && c->zero_copy_elements &&
+            cudaHostGetDevicePointer(&mapped, const_cast<double *>(elements), 0) == cudaSuccess && mapped &&
+            (reinterpret_cast<uintptr_t>(mapped) & 15u) == 0) {
+            first_src = static_cast<const double *>(mapped);
+            copy_out = c->d_el;
+        } else {
+            cudaGetLastError();
+            CU(c, cudaMemcpyAsync(c->d_el, elements, (size_t)n * 48, cudaMemcpyDefault, c->stream));
+            first_src = c->d_el;
+        }
     }
     if (n > c->acc_cap) {
         int64_t cap;
@@ -477,7 +496,8 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
             const int64_t no = std::min<int64_t>(unit_orb, n - o0);
             PropagateParams p;
             fill_common(c, p, t0);
-            p.elements = d_el + o0 * 6;
+            p.elements = (b == 0 ? first_src : d_el) + o0 * 6;
+            p.elements_copy = (b == 0 && copy_out) ? copy_out + o0 * 6 : nullptr;
             p.n_orbits = no;
             p.n_pad = (no + 31) / 32 * 32;
             p.exp = c->d_exp + first;

@@ -29,7 +29,8 @@ constexpr int kWarpsPerCta = kTileOrbits / 32;
 
 // ---- kernel 1 (+2): propagate, project, cull, compact ------------------------------------------
 struct PropagateParams {
-    const double *elements;     // [n][6] device
+    const double *elements;     // [n][6], 16-B aligned; device memory or device-mapped pinned host memory
+    double *elements_copy;      // NULL, or device [n][6]: the kernel leaves a copy of what it read
     int64_t n_orbits;           // orbits in this unit
     int64_t n_pad;              // n_orbits rounded up to 32 (mask row pitch)
     const ExpRec *exp;          // records of the unit's first exposure

@@ -66,7 +66,9 @@ constexpr int kMaxSubsteps = 12;   // sub-steps of one warm Kepler step before t
 struct __align__(128) PropSmem {
     ExpRec rec[2][kGroup];                       // 8 KB: two-slot ring of exposure groups
     uint32_t stage[kWarpsPerCta][kGroup * 32];   // 32 KB: [warp][hit] staged pixel offsets
+    double el[kTileOrbits * 6];                  // 12 KB: the tile's orbital elements (one bulk copy)
     uint64_t full[2];
+    uint64_t el_bar;
 };
 
 template <int MODE>
@@ -88,6 +90,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
     if (tid == 0) {
         mbar_init(&sm.full[0], 1);
         mbar_init(&sm.full[1], 1);
+        mbar_init(&sm.el_bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
@@ -105,11 +108,29 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
         if (g_begin + 1 < g_end) issue(g_begin + 1);
     }
 
+    // ---- the tile's elements: ONE bulk copy into shared memory.  The source may be device memory or
+    // page-locked HOST memory (dt_stack with DT_MEM_PINNED elements): the copy engine then reads the
+    // tile over PCIe in one request while earlier CTAs compute, so no separate host->device copy of
+    // the elements precedes the kernel; the first pass also leaves a device copy for later passes ----
+    const int64_t tile_base = (int64_t)blockIdx.x * kTileOrbits;
+    const int n_tile = (int)min((int64_t)kTileOrbits, p.n_orbits - tile_base);
+    if (tid == 0) {
+        const uint32_t bytes = (uint32_t)n_tile * 48u;
+        mbar_expect_tx(&sm.el_bar, bytes);
+        bulk_g2s(&sm.el[0], p.elements + tile_base * 6, bytes, &sm.el_bar);
+    }
+    mbar_wait(&sm.el_bar, 0);
+    if (p.elements_copy && blockIdx.y == 0) {
+        double2 *dst = reinterpret_cast<double2 *>(p.elements_copy + tile_base * 6);
+        const double2 *src = reinterpret_cast<const double2 *>(&sm.el[0]);
+        for (int k = tid; k < n_tile * 3; k += kTileOrbits) dst[k] = src[k];
+    }
+
     // ---- per-orbit precompute (step 1) ----
     double el[6];
     const bool in_range = orbit < p.n_orbits;
 #pragma unroll
-    for (int k = 0; k < 6; ++k) el[k] = in_range ? p.elements[orbit * 6 + k] : ((k == 0) ? -1.0 : 0.0);
+    for (int k = 0; k < 6; ++k) el[k] = in_range ? sm.el[tid * 6 + k] : ((k == 0) ? -1.0 : 0.0);
     const Orbit o = orbit_setup(el, p.gm, p.cos_eps, p.sin_eps, p.inv_c, p.tan_fov);
 
     Kepler K;

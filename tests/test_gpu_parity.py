@@ -344,3 +344,43 @@ def test_fp64_peak_probe_runs():
     tf = dt.dt_fp64_peak(0)
     print("FP64 DFMA peak: %.2f TFLOP/s" % tf)
     assert 5.0 < tf < 100.0
+
+
+def test_pinned_elements_zero_copy_matches_device_path():
+    """dt_stack with page-locked host elements (kernel 1 bulk-copies each tile straight from host
+    memory and leaves the device copy for the later exposure units and the finalisation) and
+    caller-supplied pinned outputs == the device-pointer path, bit for bit; several orbit tiles with a
+    ragged tail, two exposure units (streaming forces more than one pass over the orbits)."""
+    dt = _dt()
+    sc = _scene("mba_focused")
+    cfg = sc.cfg
+    flux, _ = _planes(sc, 0)
+    el = sc.elements()[:5003]
+    el[17, 0] = -1.0                                   # an invalid orbit rides along
+    n = el.shape[0]
+    el_pin = torch.from_numpy(el.copy()).pin_memory()
+    out = (torch.empty(n, dtype=torch.float64).pin_memory(), torch.empty(n, dtype=torch.int32).pin_memory())
+    res = {}
+    for mode in ("device", "pinned", "pinned_streamed"):
+        kw = {}
+        if mode == "pinned_streamed":
+            kw = dict(flags=1, hbm_budget_bytes=2 * 40 * cfg.plane_pixels * 4)   # 40-exposure batches
+        with dt.Tracker.from_scene(sc, **kw) as trk:
+            if mode == "pinned_streamed":
+                fp = torch.from_numpy(flux).pin_memory()
+                trk.load_image_batch(0, fp)
+            else:
+                trk.load_image_batch(0, flux)
+            if mode == "device":
+                s, h = trk.stack(torch.from_numpy(el).cuda(), sc.t0)
+                res[mode] = (s.cpu().numpy(), h.cpu().numpy())
+            else:
+                s, h = trk.stack(el_pin, sc.t0, out=out)
+                assert s is out[0] and h is out[1]
+                res[mode] = (s.numpy().copy(), h.numpy().copy())
+                if mode == "pinned_streamed":
+                    assert trk.stats()["n_image_batches"] >= 2
+    for mode in ("pinned", "pinned_streamed"):
+        assert np.array_equal(res[mode][1], res["device"][1])
+        assert np.array_equal(res[mode][0], res["device"][0], equal_nan=True)
+    assert res["device"][1][17] == -1 and np.isnan(res["device"][0][17])
