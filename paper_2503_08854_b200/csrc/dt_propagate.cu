@@ -61,7 +61,7 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 #ifndef DT_K1_MIN_CTAS
 #define DT_K1_MIN_CTAS 2           // resident CTAs per SM kernel 1 is compiled for (register budget)
 #endif
-constexpr int kMaxSubsteps = 12;   // sub-steps of one warm Kepler step before the cold solve is cheaper
+constexpr int kMaxSubsteps = 6;    // wide sub-steps of one Kepler step before the cold solve is cheaper
 
 struct __align__(128) PropSmem {
     ExpRec rec[2][kGroup];                       // 8 KB: two-slot ring of exposure groups
@@ -163,21 +163,24 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 if (__all_sync(0xffffffffu, ok)) {
                     K = Kw;
                 } else {
-                    // some lane's step is too long for one warm step (long gap, or close to the
-                    // perihelion of an eccentric orbit): split it into equal sub-steps in M, the
-                    // count warp-uniform; only when that would take too many, solve cold
+                    // some lane's step is too long for the narrow warm step (long gap, or close to
+                    // the perihelion of an eccentric orbit): take one wide warm step, or split the
+                    // step into equal wide sub-steps in M (count warp-uniform); only when that
+                    // would take too many, solve cold
                     bool solved = false;
                     if (have_state) {
                         const float r = __uint_as_float(
                             __reduce_max_sync(0xffffffffu, __float_as_uint(kepler_warm_need(o.e, K, M))));
-                        if (r < (float)kMaxSubsteps / 1.5f) {       // false for NaN
-                            const int ns = max(2, (int)ceilf(1.5f * r));
+                        // r <= 1 is the wide step's own domain; the margins leave room for the
+                        // coefficients growing on the way to a perihelion (every sub-step re-checks)
+                        if (r < (float)kMaxSubsteps / 1.3f) {       // false for NaN
+                            const int ns = (r <= 0.8f) ? 1 : (int)ceilf(1.3f * r);
                             const double M_from = K.M, dMs = (M - M_from) / (double)ns;
                             Kepler Kc = K;
                             bool good = true;
                             for (int sidx = 1; sidx <= ns; ++sidx) {
                                 bool oks;
-                                Kc = kepler_warm(o.e, Kc, (sidx == ns) ? M : fma(dMs, (double)sidx, M_from), oks);
+                                Kc = kepler_warm_wide(o.e, Kc, (sidx == ns) ? M : fma(dMs, (double)sidx, M_from), oks);
                                 good = good && oks;
                             }
                             if (__all_sync(0xffffffffu, good)) {
