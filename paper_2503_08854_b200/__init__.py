@@ -64,7 +64,7 @@ def lib():
     """The loaded C-ABI library; built in-tree with nvcc on first use.  Raises when unavailable."""
     global _lib
     if _lib is None:
-        path = _build.build()
+        path = os.environ.get("DTRACK_LIB") or _build.build()   # DTRACK_LIB: a prebuilt library
         if not os.path.exists(path):
             raise RuntimeError("libdtrack.so is missing and could not be built; there is no CPU fallback")
         L = C.CDLL(path)

@@ -5,7 +5,7 @@
 // compacted hits leave the SM, cf. PAPER.md:202 where the paper stores "tens of bytes for each
 // pair").
 //
-// Mapping: one orbit per thread (32 orbits per warp, 256 per CTA); the thread walks the unit's
+// Mapping: one orbit per thread (32 orbits per warp, kTileOrbits = 128 per CTA, 4 CTAs per SM); the thread walks the unit's
 // exposures in time order carrying its Kepler state, so consecutive solves are warm-started.
 // Exposure records (128 B each) are staged group by group (32 exposures = 4 KB) into shared memory
 // by 1-D TMA bulk copies (cp.async.bulk, SASS UBLKCP) on a two-slot mbarrier ring; every lane
@@ -59,14 +59,14 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 }
 
 #ifndef DT_K1_MIN_CTAS
-#define DT_K1_MIN_CTAS 2           // resident CTAs per SM kernel 1 is compiled for (register budget)
+#define DT_K1_MIN_CTAS 4           // resident CTAs per SM kernel 1 is compiled for (register budget)
 #endif
 constexpr int kMaxSubsteps = 6;    // wide sub-steps of one Kepler step before the cold solve is cheaper
 
 struct __align__(128) PropSmem {
     ExpRec rec[2][kGroup];                       // 8 KB: two-slot ring of exposure groups
-    uint32_t stage[kWarpsPerCta][kGroup * 32];   // 32 KB: [warp][hit] staged pixel offsets
-    double el[kTileOrbits * 6];                  // 12 KB: the tile's orbital elements (one bulk copy)
+    uint32_t stage[kWarpsPerCta][kGroup * 32];   // 4 KB per warp: [warp][hit] staged pixel offsets
+    double el[kTileOrbits * 6];                  // 48 B per orbit: the tile's elements (one bulk copy)
     uint64_t full[2];
     uint64_t el_bar;
 };
