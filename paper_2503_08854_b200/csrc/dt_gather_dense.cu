@@ -37,7 +37,7 @@ __device__ __forceinline__ void red_add_relaxed(int *p, int v)
 // Shared memory of one CTA: (S, Wt) [T][kGatherThreads] double2, cnt [T][kGatherThreads] int32
 // (accumulators, lane-private), arrive [n_local] int, done_upto int (lock-step throttle).
 template <bool PLANE_VAR>
-__global__ void __launch_bounds__(kGatherThreads, 2) k_gather_dense(const GatherParams p)
+__global__ void __launch_bounds__(kGatherThreads, kGatherCtasPerSm) k_gather_dense(const GatherParams p)
 {
     if (!gather_is_dense(p)) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -208,7 +208,7 @@ static cudaError_t dense_geometry(int64_t n_pad, int32_t n_groups, int device, i
     }
     constexpr int n_warps = kGatherThreads / 32;
     const int64_t n_tiles = n_pad >> 5;
-    const int max_ctas = sm_count * 2;                 // __launch_bounds__(kGatherThreads, 2)
+    const int max_ctas = sm_count * kGatherCtasPerSm;
     int64_t ctas = (n_tiles + n_warps - 1) / n_warps;
     if (ctas > max_ctas) ctas = max_ctas;
     if (ctas < 1) ctas = 1;
