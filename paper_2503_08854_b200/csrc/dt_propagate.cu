@@ -159,7 +159,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
             if (WARM) {
                 bool ok = false;
                 Kepler Kw = K;
-                if (have_state) Kw = kepler_warm(o.e, K, M, ok);
+                if (have_state) Kw = kepler_warm<3>(o.e, K, M, ok);
                 if (__all_sync(0xffffffffu, ok)) {
                     K = Kw;
                 } else {
@@ -226,7 +226,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 Kepler K1;
                 if (WARM) {
                     bool ok1;
-                    K1 = kepler_warm(o.e, K, M1, ok1);
+                    K1 = kepler_warm<2>(o.e, K, M1, ok1);
                     if (!__all_sync(0xffffffffu, ok1)) K1 = kepler_newton_from(o.e, K, M1);
                 } else {
                     K1 = kepler_newton_from(o.e, K, M1);
