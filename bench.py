@@ -31,12 +31,12 @@ import dtsynth as ds  # noqa: E402
 METRIC = "orbit-exposure pairs/sec (propagate+project+gather+stack)"
 UNIT = "pairs/s"
 # FP64-pipe instructions kernel 1 issues per pair on its two paths,
-# measured with ncu smsp__inst_executed_pipe_fp64.sum on configs[1] (profiles/r1c_final.md): 70.0 per pair
-# with the pre-cull (0.02 % of the pairs refined) and 140.0 per pair with DT_FLAG_NO_PRECULL (every pair
+# measured with ncu smsp__inst_executed_pipe_fp64.sum on configs[1] (profiles/r1c_final.md): 66.0 per pair
+# with the pre-cull (0.02 % of the pairs refined) and 130.0 per pair with DT_FLAG_NO_PRECULL (every pair
 # refined; that mode has no cone test, ~6 instructions).  Other workloads take longer Kepler paths
 # (wide steps on NEO), so the model under-counts their work: their `frac` is a lower bound.
-FP64_SLOTS_COARSE = 70.0     # order-3 warm Kepler step + geometric position + cone test (every pair)
-FP64_SLOTS_REFINE = 76.0     # light-time re-solve + projection + footprint test (refined pairs only)
+FP64_SLOTS_COARSE = 66.0     # order-3 warm Kepler step + geometric position + cone test (every pair)
+FP64_SLOTS_REFINE = 70.0     # light-time re-solve + projection + footprint test (refined pairs only)
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_propagate<3> launch on configs[1], from the
 # `ncu --set full` capture summarised in profiles/r1b_gather.md (48.52 MB + 19.53 MB)
 K1_TRAFFIC_BYTES_SMALL_MBA = 68.05e6
@@ -400,7 +400,7 @@ def main():
         refined_frac = stats["refined_pairs"] / max(stats["pairs"], 1)
         slots = FP64_SLOTS_COARSE + refined_frac * FP64_SLOTS_REFINE
         if args.flags & 4:
-            slots = 140.0
+            slots = 130.0
         achieved_tf = 2.0 * slots * pairs_per_launch / (ms_k1 * 1e-3) * 1e-12
         roofline = {"bound": "alu", "kernel": "k_propagate", "achieved": achieved_tf, "peak": peak_tf,
                     "unit": "TFLOP/s", "frac": achieved_tf / peak_tf if peak_tf else None,

@@ -79,7 +79,8 @@ __device__ __forceinline__ Orbit orbit_setup(const double el_in[6], double gm, d
 }
 
 // ---- small fp64 helpers: MUFU seed + Newton, no slow-path branches ---------------------------------
-// 1/x for normal, finite x; relative error ~1e-12 after two iterations (three: ~1 ulp).
+// 1/x for normal, finite x; measured on B200: MUFU seed 9.8e-7 relative, 9.7e-13 after one
+// iteration, correctly rounded after two.
 template <int ITERS>
 __device__ __forceinline__ double rcp_nr(double x)
 {
@@ -248,13 +249,15 @@ __device__ __forceinline__ Kepler kepler_warm_tail(double e, const Kepler &K0, d
     }
     const double st = fma(th * z, ps, th);
     const double cm = z * pc;
-    const double s1 = K0.s + fma(K0.c, st, K0.s * cm);
-    const double c1 = K0.c + fma(-K0.s, st, K0.c * cm);
+    const double s1 = fma(K0.s, cm, fma(K0.c, st, K0.s));
+    const double c1 = fma(K0.c, cm, fma(-K0.s, st, K0.c));
     const double u1 = K0.u + (th - dM);
-    // Newton polish: f1 = u1 - e s1, 1/g1 from one Newton step on rg
+    // Newton polish: f1 = u1 - e s1, and 1/g1 from its own MUFU seed + one Newton step (1e-12
+    // relative, measured; d <= ~1e-6).  One Newton step from rg instead leaves ((g1 - g)/g)^2 of d,
+    // up to 1.3e-10 rad at e = 0.9 next to a perihelion.
     const double f1 = fma(-e, s1, u1);
     const double g1 = fma(-e, c1, 1.0);
-    const double rg1 = rg * fma(-g1, rg, 2.0);
+    const double rg1 = rcp_nr<1>(g1);
     const double d = -f1 * rg1;
     Kepler K;
     K.M = Mn;
@@ -274,7 +277,7 @@ __device__ __forceinline__ Kepler kepler_warm(double e, const Kepler &K0, double
     const double es = e * K0.s, ec = e * K0.c;
     const double f0 = (K0.u - es) - dM;
     const double g = 1.0 - ec;
-    const double rg = rcp_nr<2>(g);
+    const double rg = rcp_nr<1>(g);          // 1e-12 relative: the polish removes what it costs theta
     const double x = -f0 * rg;
     const double a2 = 0.5 * es * rg;
     const double ax = fabs(x), axa2 = fabs(x * a2);

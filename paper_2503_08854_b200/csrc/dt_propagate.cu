@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 qz = fma(o.Az, X1, fma(o.Bz, K1.s, -x.Rz));
                 // ---- step 6: gnomonic projection (vector form) + pixelise ----
                 const double D = fma(qx, x.tx, fma(qy, x.ty, qz * x.tz));
-                const double inv = WARM ? rcp_nr<3>(D) : 1.0 / D;
+                const double inv = WARM ? rcp_nr<2>(D) : 1.0 / D;
                 const double xe = fma(qx, x.ex, fma(qy, x.ey, qz * x.ez));
                 const double xn = fma(qx, x.nx, fma(qy, x.ny, qz * x.nz));
                 xpix = fma(xe, inv, p.cx);
