@@ -384,3 +384,53 @@ def test_pinned_elements_zero_copy_matches_device_path():
         assert np.array_equal(res[mode][1], res["device"][1])
         assert np.array_equal(res[mode][0], res["device"][0], equal_nan=True)
     assert res["device"][1][17] == -1 and np.isnan(res["device"][0][17])
+
+
+@pytest.mark.parametrize("flags", [0, 2], ids=["warm", "cold"])
+def test_perihelion_stress_all_kepler_paths(flags):
+    """Eccentric orbits (e up to 0.9) whose perihelion passages fall inside the exposure span, with
+    exposure gaps from minutes to weeks: the warm step at its three orders, the wide step, wide
+    sub-steps and the cold solve are all taken (counted), and every sky position / pixel coordinate
+    must still match the oracle (1e-10 rad; continuous pixel coordinates to 1e-6 px; pixel indices
+    exact off the guard band).  Eight families of orbits, each around a guide the tangent points track in
+    turn, keep an eighth of all pairs near-field."""
+    dt = _dt()
+    rng = np.random.default_rng(11)
+    N, n, W, H = 200, 2048, 512, 512
+    gaps = np.concatenate([rng.uniform(0.003, 0.05, 60), rng.uniform(0.05, 1.0, 80), rng.uniform(1.0, 20.0, 59)])
+    rng.shuffle(gaps)
+    t = np.concatenate([[0.0], np.cumsum(gaps)])
+    G = 8                                                    # guide orbits; families of n / G members
+    ga = rng.uniform(0.8, 1.6, G)
+    ge = np.concatenate([rng.uniform(0.88, 0.9, G // 2), rng.uniform(0.6, 0.88, G - G // 2)])
+    period = 2 * np.pi / np.sqrt(ds.GM_SUN / ga ** 3)
+    t_peri = rng.uniform(0.2, 0.8, G) * t[-1]                # a perihelion passage inside the span
+    guides = np.stack([ga, ge, rng.uniform(0, 0.5, G), rng.uniform(0, 2 * np.pi, G), rng.uniform(0, 2 * np.pi, G),
+                       -2 * np.pi / period * t_peri], 1)
+    fam = np.repeat(np.arange(G), n // G)
+    el = guides[fam] + rng.uniform(-1, 1, (n, 6)) * np.array([1e-5, 1e-5, 3e-5, 3e-5, 3e-5, 3e-5])
+    el[::n // G] = guides                                    # member 0 of each family is the guide itself
+    obs = ds.observer_ecliptic(t)
+    probe = oracle.Survey(t, obs, np.zeros(N), np.zeros(N), W, H, ds.PIXEL_SCALE, ds.GM_SUN, ds.C_AU_PER_DAY,
+                          ds.OBLIQUITY, 0, np.ones(N))
+    gr = oracle.project(probe, guides, 0.0)["radec"]         # [G, N, 2]
+    track = gr[np.arange(N) % G, np.arange(N)]               # exposure j looks at guide j mod G
+    sv = oracle.Survey(t, obs, track[:, 0], track[:, 1], W, H, ds.PIXEL_SCALE, ds.GM_SUN, ds.C_AU_PER_DAY,
+                       ds.OBLIQUITY, 0, np.ones(N))
+    ref = oracle.project(sv, el, 0.0)
+    with dt.Tracker(t, obs, track[:, 0], track[:, 1], W, H, ds.PIXEL_SCALE, variance_mode=0, var_scalar=np.ones(N),
+                    flags=flags) as trk:
+        out = trk.project(el, 0.0)
+        n_bad = _compare_project(out, ref)
+        trk.load_image_batch(0, np.ones((N, H, W), np.float32))
+        snr, hits = trk.stack(el, 0.0)
+        st = trk.stats()
+    # a guide is seen in every exposure that tracks it; unit images: SNR = sqrt(hits)
+    assert hits[0] >= N // G and abs(snr[0] - math.sqrt(hits[0])) < 1e-12
+    near = (np.abs(ref["xy"]) < 1e5).all(-1)
+    assert near.sum() > 0.1 * n * N                          # the 1e-6 px comparison covered many pairs
+    if flags == 0:
+        assert st["substep_solves"] > 0.05 * n * N, st          # wide steps / sub-steps were exercised
+        assert 0 < st["cold_solves"] < 0.5 * n * N, st          # and so was the cold solve, but rarely
+    print("perihelion stress: flagged pixel mismatches %d, substep %d, cold %d of %d pairs" %
+          (n_bad, st["substep_solves"], st["cold_solves"], n * N))
