@@ -38,8 +38,8 @@ UNIT = "pairs/s"
 FP64_SLOTS_COARSE = 66.0     # order-3 warm Kepler step + geometric position + cone test (every pair)
 FP64_SLOTS_REFINE = 70.0     # light-time re-solve + projection + footprint test (refined pairs only)
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_propagate<3> launch on configs[1], from the
-# `ncu --set full` capture summarised in profiles/r1b_gather.md (48.52 MB + 19.53 MB)
-K1_TRAFFIC_BYTES_SMALL_MBA = 68.05e6
+# `ncu --set full` capture summarised in profiles/r1c_final.md (48.11 MB + 19.42 MB)
+K1_TRAFFIC_BYTES_SMALL_MBA = 67.54e6
 
 
 def parse_args():
@@ -406,7 +406,7 @@ def main():
                     "unit": "TFLOP/s", "frac": achieved_tf / peak_tf if peak_tf else None,
                     "traffic": K1_TRAFFIC_BYTES_SMALL_MBA if (cfg.name == "small_mba" and not args.orbits and
                                                               not args.exposures and not args.flags) else None,
-                    "traffic_unit": "bytes per launch (ncu dram read + write, profiles/r1b_gather.md)",
+                    "traffic_unit": "bytes per launch (ncu dram read + write, profiles/r1c_final.md)",
                     "peak_source": "dt_fp64_peak DFMA probe measured in this run (MEASURED_PEAKS.json has no FP64 figure)",
                     "fp64_slots_per_pair": slots, "refined_fraction": refined_frac,
                     "ms_per_launch": ms_k1, "share_of_step": float(np.mean(ms_prop)) / ms_step}
