@@ -267,27 +267,50 @@ __device__ __forceinline__ Kepler kepler_warm_tail(double e, const Kepler &K0, d
     return K;
 }
 
+// The part of the warm step that comes before its order is known: first-order step x and a2.
+struct WarmPre {
+    double dM, es, ec, rg, x, a2, ax, axa2;
+};
+__device__ __forceinline__ WarmPre kepler_warm_pre(double e, const Kepler &K0, double Mn)
+{
+    WarmPre w;
+    w.dM = Mn - K0.M;
+    w.es = e * K0.s;
+    w.ec = e * K0.c;
+    const double f0 = (K0.u - w.es) - w.dM;
+    w.rg = rcp_nr<1>(1.0 - w.ec);            // 1e-12 relative: the polish removes what it costs theta
+    w.x = -f0 * w.rg;
+    w.a2 = 0.5 * w.es * w.rg;
+    w.ax = fabs(w.x);
+    w.axa2 = fabs(w.x * w.a2);
+    return w;
+}
+template <int ORDER>
+__device__ __forceinline__ bool kepler_warm_in_domain(const WarmPre &w)
+{
+    const double *C = kWarmC;
+    if (ORDER == 4) return (w.ax <= C[9]) && (w.axa2 <= C[10]);
+    if (ORDER == 3) return (w.ax <= C[11]) && (w.axa2 <= C[12]);
+    return (w.ax <= C[13]) && (w.axa2 <= C[14]);
+}
+template <int ORDER>
+__device__ __forceinline__ Kepler kepler_warm_finish(double e, const Kepler &K0, double Mn, const WarmPre &w)
+{
+    return kepler_warm_tail<ORDER>(e, K0, Mn, w.dM, w.es, w.ec, w.rg, w.x, w.a2);
+}
+
 // LOW = 3 for the exposure-to-exposure step, 2 for the light-time re-solve: the warp takes the cheaper
 // order when every lane's step is inside its domain (one vote), else ORDER 4.  All 32 lanes must call.
 template <int LOW>
 __device__ __forceinline__ Kepler kepler_warm(double e, const Kepler &K0, double Mn, bool &ok)
 {
-    const double *C = kWarmC;
-    const double dM = Mn - K0.M;
-    const double es = e * K0.s, ec = e * K0.c;
-    const double f0 = (K0.u - es) - dM;
-    const double g = 1.0 - ec;
-    const double rg = rcp_nr<1>(g);          // 1e-12 relative: the polish removes what it costs theta
-    const double x = -f0 * rg;
-    const double a2 = 0.5 * es * rg;
-    const double ax = fabs(x), axa2 = fabs(x * a2);
-    const bool low = (LOW == 3) ? (ax <= C[11] && axa2 <= C[12]) : (ax <= C[13] && axa2 <= C[14]);
-    if (__all_sync(0xffffffffu, low)) {
+    const WarmPre w = kepler_warm_pre(e, K0, Mn);
+    if (__all_sync(0xffffffffu, kepler_warm_in_domain<LOW>(w))) {
         ok = true;
-        return kepler_warm_tail<LOW>(e, K0, Mn, dM, es, ec, rg, x, a2);
+        return kepler_warm_finish<LOW>(e, K0, Mn, w);
     }
-    ok = (ax <= C[9]) && (axa2 <= C[10]);
-    return kepler_warm_tail<4>(e, K0, Mn, dM, es, ec, rg, x, a2);
+    ok = kepler_warm_in_domain<4>(w);
+    return kepler_warm_finish<4>(e, K0, Mn, w);
 }
 
 // Wide warm step: the same 4th-order series start, but for steps 7.5 times longer (|x| <= 0.3,
