@@ -334,7 +334,7 @@ def main():
 
     if args.gather_only:
         hbm, src = measured_hbm_peak()
-        print(json.dumps({"gather_roofline": {"bound": "hbm", "kernel": "k_gather_stack", "peak_source": src,
+        print(json.dumps({"gather_roofline": {"bound": "hbm", "kernel": "k_gather_dense / k_gather_sparse", "peak_source": src,
                                               "regimes": gather_bench(dt, trk, cfg, dev, hbm, args.gather_reps,
                                                                       pick_regimes(args))}}))
         trk.close()
@@ -426,7 +426,7 @@ def main():
                 "wall_s_timed_region": wall}
         if not args.no_gather_bench:
             hbm, src = measured_hbm_peak()
-            line["gather_roofline"] = {"bound": "hbm", "kernel": "k_gather_stack", "peak_source": src,
+            line["gather_roofline"] = {"bound": "hbm", "kernel": "k_gather_dense / k_gather_sparse", "peak_source": src,
                                        "regimes": gather_bench(dt, trk, cfg, dev, hbm, args.gather_reps,
                                                                pick_regimes(args))}
         if not args.no_cpu_baseline:
