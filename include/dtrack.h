@@ -109,6 +109,8 @@ typedef struct {
     float ms_finalize;         /* SNR finalisation                                                */
     int32_t launches;          /* kernels launched by the call                                    */
     int32_t propagate_launches, gather_launches;
+    int32_t image_zero_copy;   /* 1 when a streamed survey was gathered straight from the pinned host     */
+                               /* planes (few hits) instead of being copied batch by batch               */
 } dt_stats;
 
 /*

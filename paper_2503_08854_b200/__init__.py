@@ -54,7 +54,7 @@ class dt_stats(C.Structure):
                 ("substep_solves", C.c_int64), ("h2d_image_bytes", C.c_int64), ("streamed", C.c_int32), ("n_image_batches", C.c_int32),
                 ("ms_total", C.c_float), ("ms_propagate", C.c_float), ("ms_gather", C.c_float),
                 ("ms_finalize", C.c_float), ("launches", C.c_int32), ("propagate_launches", C.c_int32),
-                ("gather_launches", C.c_int32)]
+                ("gather_launches", C.c_int32), ("image_zero_copy", C.c_int32)]
 
 
 _lib = None

@@ -70,6 +70,8 @@ struct dt_context {
     int32_t gather_window = 1;                          // exposures the slowest and fastest CTA may be apart
     int32_t gather_lockstep = -1;                       // -1: decided on the device from the hit density
     int32_t gather_ld_cached = 1;
+    int32_t stream_zero_copy = -1;                      // DT_STREAM_ZERO_COPY: -1 decide from a probe, 0 never, 1 always
+    const float **d_flux_ptrs = nullptr, **d_var_ptrs = nullptr;   // [N] device-mapped pinned planes (zero-copy gather)
     bool zero_copy_elements = true;                     // DT_ZERO_COPY=0: copy pinned elements to the device first
     std::vector<cudaEvent_t> ev_pool;                   // timing events
 
@@ -137,6 +139,8 @@ void free_all(dt_context *c)
     cudaFree(c->d_offsets);
     cudaFree(c->d_counters);
     cudaFree(c->d_progress);
+    cudaFree((void *)c->d_flux_ptrs);
+    cudaFree((void *)c->d_var_ptrs);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     topk_free(c->topk);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
@@ -278,6 +282,7 @@ int dt_create(const dt_survey *s, dt_context **out)
         if (cudaMalloc((void **)&c->d_counters, 8 * sizeof(unsigned long long)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
         if (cudaMalloc((void **)&c->d_progress, (size_t)(kMaxUnitExposures + kGroup) * kProgressStride * sizeof(int)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
         c->gather_window = pick_gather_window(c);
+        if (const char *env = getenv("DT_STREAM_ZERO_COPY")) c->stream_zero_copy = atoi(env) < 0 ? -1 : (atoi(env) ? 1 : 0);
         if (const char *env = getenv("DT_ZERO_COPY")) c->zero_copy_elements = atoi(env) != 0;
         if (const char *env = getenv("DT_GATHER_L1")) c->gather_ld_cached = atoi(env) ? 1 : 0;
         if (const char *env = getenv("DT_GATHER_LOCKSTEP")) c->gather_lockstep = atoi(env) < 0 ? -1 : (atoi(env) ? 1 : 0);
@@ -475,7 +480,67 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
         return DT_OK;
     };
 
-    if (c->streaming) {
+    // ---- streaming mode, few hits: gather straight from the page-locked host planes (zero-copy) ----
+    // A survey larger than HBM costs its whole size over PCIe per pass when it is streamed (268 GB at
+    // 55 GB/s = 4.9 s on configs[2]) although a blind search touches a few pixels per exposure (the
+    // paper's own observation, "extremely sparse").  When the planes are device-mappable
+    // and a probe (kernel 1 on the first orbit unit and exposure batch) predicts that the gathers
+    // would move less than 5 % of the bytes streaming would, no image is copied at all and the sparse
+    // gather reads the hit pixels over PCIe.  Same pixels, same arithmetic: bit-identical results.
+    bool zero_copy_images = false;
+    if (c->streaming && c->stream_zero_copy != 0) {
+        std::vector<const float *> hf(c->N), hv(c->N, nullptr);
+        bool mappable = true;
+        for (int32_t j = 0; j < c->N && mappable; ++j) {
+            void *d = nullptr;
+            mappable = cudaHostGetDevicePointer(&d, const_cast<float *>(c->h_flux[j]), 0) == cudaSuccess && d;
+            hf[j] = static_cast<const float *>(d);
+            if (mappable && c->var_mode == 1) {
+                mappable = cudaHostGetDevicePointer(&d, const_cast<float *>(c->h_var[j]), 0) == cudaSuccess && d;
+                hv[j] = static_cast<const float *>(d);
+            }
+        }
+        if (!mappable) {
+            cudaGetLastError();
+        } else {
+            if (!c->d_flux_ptrs) CU(c, cudaMalloc((void **)&c->d_flux_ptrs, sizeof(float *) * (size_t)c->N));
+            if (!c->d_var_ptrs) CU(c, cudaMalloc((void **)&c->d_var_ptrs, sizeof(float *) * (size_t)c->N));
+            CU(c, cudaMemcpyAsync((void *)c->d_flux_ptrs, hf.data(), sizeof(float *) * (size_t)c->N,
+                                  cudaMemcpyHostToDevice, c->stream));
+            CU(c, cudaMemcpyAsync((void *)c->d_var_ptrs, hv.data(), sizeof(float *) * (size_t)c->N,
+                                  cudaMemcpyHostToDevice, c->stream));
+            if (c->stream_zero_copy == 1) {
+                zero_copy_images = true;
+            } else {
+                const int64_t no = std::min<int64_t>(unit_orb, n);
+                const int32_t ne = std::min<int32_t>(unit_exp, c->N);
+                PropagateParams p;
+                fill_common(c, p, t0);
+                p.elements = first_src;
+                p.n_orbits = no;
+                p.n_pad = (no + 31) / 32 * 32;
+                p.exp = c->d_exp;
+                p.n_exp = ne;
+                p.groups_per_split = pick_groups_per_split(no, ne);
+                p.mask = c->d_mask;
+                p.base = c->d_base;
+                p.offsets = c->d_offsets;
+                p.counters = c->d_counters;
+                CU(c, launch_propagate(p, mode, c->stream));
+                st.propagate_launches += 1;
+                unsigned long long probe_hits = 0;
+                CU(c, cudaMemcpyAsync(&probe_hits, c->d_counters, sizeof probe_hits, cudaMemcpyDeviceToHost, c->stream));
+                CU(c, cudaStreamSynchronize(c->stream));
+                CU(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+                const double planes = (c->var_mode == 1) ? 2.0 : 1.0;
+                const double gathers = (double)probe_hits / ((double)no * ne) * (double)n * c->N * planes;
+                zero_copy_images = gathers * 128.0 < 0.05 * (double)c->N * (double)c->plane * 4.0 * planes;
+            }
+        }
+    }
+    st.image_zero_copy = zero_copy_images ? 1 : 0;
+
+    if (c->streaming && !zero_copy_images) {
         // the copy stream must not start before earlier work on the context stream that may still
         // read the slots (a previous dt_stack) has been ordered: previous calls synchronise, so
         // only the free events of this call matter
@@ -487,7 +552,7 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
     for (int b = 0; b < n_batches; ++b) {
         const int slot = b & 1;
         const int32_t first = b * unit_exp, n_exp = std::min<int32_t>(unit_exp, c->N - first);
-        if (c->streaming && b + 1 < n_batches) {
+        if (c->streaming && !zero_copy_images && b + 1 < n_batches) {
             rc = issue_copy(b + 1);
             if (rc != DT_OK) return rc;
         }
@@ -514,7 +579,7 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
             st.propagate_launches += 1;
             CU(c, cudaEventRecord(ev_at(3 * unit_idx + 1), c->stream));
 
-            if (c->streaming && !waited) {
+            if (c->streaming && !zero_copy_images && !waited) {
                 CU(c, cudaStreamWaitEvent(c->stream, c->ev_ready[slot], 0));
                 waited = true;
             }
@@ -527,7 +592,10 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
             g.mask = c->d_mask;
             g.base = c->d_base;
             g.offsets = c->d_offsets;
-            if (c->streaming) {
+            if (zero_copy_images) {
+                g.flux_ptrs = c->d_flux_ptrs;
+                g.var_ptrs = (c->var_mode == 1) ? c->d_var_ptrs : nullptr;
+            } else if (c->streaming) {
                 g.flux = c->d_buf_flux[slot] - (int64_t)first * c->plane;
                 g.var = (c->var_mode == 1) ? c->d_buf_var[slot] - (int64_t)first * c->plane : nullptr;
             } else {
@@ -542,14 +610,14 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
             g.progress = c->d_progress;
             g.window = c->gather_window;
             g.n_hits_dev = c->d_counters;            // the unit's hit allocator, final after kernel 1
-            g.lockstep_mode = c->gather_lockstep;
+            g.lockstep_mode = zero_copy_images ? 0 : c->gather_lockstep;
             g.ld_cached = c->gather_ld_cached;
             CU(c, launch_gather(g, c->device, c->stream));
-            st.gather_launches += (c->gather_lockstep < 0) ? 2 : 1;   // sparse + dense schedule, one of them returns at once
+            st.gather_launches += (g.lockstep_mode < 0) ? 2 : 1;   // sparse + dense schedule, one of them returns at once
             CU(c, cudaEventRecord(ev_at(3 * unit_idx + 2), c->stream));
             unit_idx += 1;
         }
-        if (c->streaming) {
+        if (c->streaming && !zero_copy_images) {
             CU(c, cudaEventRecord(c->ev_free[slot], c->stream));
             c->ev_free_recorded[slot] = true;
         }

@@ -69,6 +69,10 @@ struct GatherParams {
     const uint32_t *offsets;
     const float *flux;          // plane of ABSOLUTE exposure j at flux + j * plane
     const float *var;           // same indexing; NULL in scalar mode
+    // zero-copy mode (sparse schedule only): per-exposure plane pointers, absolute index, device-mapped
+    // page-locked HOST memory; flux / var above are NULL then
+    const float *const *flux_ptrs;
+    const float *const *var_ptrs;
     const ExpRec *exp_all;      // all exposure records (scalar variance), absolute index
     int64_t plane;              // pixels per plane
     double *S, *Wt;             // [n] running sums (read-modify-write once per launch)

@@ -14,6 +14,8 @@
 //     lanes below).  Every lane then walks ITS OWN hits in ascending exposure order, four in
 //     flight, so all lanes stay busy however few exposures a block touches.  Bound: the rate of
 //     random DRAM accesses (no reuse to exploit when hits are sparse).
+//     In streaming mode with few hits it can also read the pixels straight from the page-locked host
+//     planes (zero-copy), so that a survey larger than HBM need not be streamed at all.
 //   * k_gather_dense (dt_gather_dense.cu): one persistent wave sweeping the exposures in lock-step so
 //     that the planes being gathered from stay L2-resident while every orbit of the unit reads them.
 // Both accumulate S += f/v, Wt += 1/v per orbit in ascending exposure order in a lane-private
@@ -90,13 +92,19 @@ __global__ void __launch_bounds__(kSparseThreads) k_gather_sparse(const GatherPa
                 f[q] = 0.f;
                 vv[q] = 1.f;
                 if (have[q]) {
-                    const int64_t a = (j0 + jj[q]) * p.plane + off[q];
-                    if (cached) {
-                        f[q] = ld_pixel_cached(p.flux + a);
-                        if (PLANE_VAR) vv[q] = ld_pixel_cached(p.var + a);
+                    if (p.flux_ptrs) {
+                        // zero-copy: the pixel comes straight from page-locked host memory over PCIe
+                        f[q] = ld_pixel_cached(p.flux_ptrs[j0 + jj[q]] + off[q]);
+                        if (PLANE_VAR) vv[q] = ld_pixel_cached(p.var_ptrs[j0 + jj[q]] + off[q]);
                     } else {
-                        f[q] = ld_pixel_stream(p.flux + a);
-                        if (PLANE_VAR) vv[q] = ld_pixel_stream(p.var + a);
+                        const int64_t a = (j0 + jj[q]) * p.plane + off[q];
+                        if (cached) {
+                            f[q] = ld_pixel_cached(p.flux + a);
+                            if (PLANE_VAR) vv[q] = ld_pixel_cached(p.var + a);
+                        } else {
+                            f[q] = ld_pixel_stream(p.flux + a);
+                            if (PLANE_VAR) vv[q] = ld_pixel_stream(p.var + a);
+                        }
                     }
                 }
             }
@@ -131,7 +139,7 @@ cudaError_t launch_gather(const GatherParams &p_in, int device, cudaStream_t str
     if (p.window < 1) p.window = 1;
     if (p.lockstep_mode != 1) {
         const unsigned blocks = (unsigned)((p.n_pad + kSparseThreads - 1) / kSparseThreads);
-        if (p.var)
+        if (p.var || p.var_ptrs)
             k_gather_sparse<true><<<blocks, kSparseThreads, 0, stream>>>(p);
         else
             k_gather_sparse<false><<<blocks, kSparseThreads, 0, stream>>>(p);

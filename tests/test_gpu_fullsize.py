@@ -183,22 +183,36 @@ def test_full_size_lsst_streamed():
     for q in range(POOL):
         flux_pool[q].copy_(ds.noise_plane_t(cfg, q, dev))
         var_pool[q].fill_(float(scene.var_scalar[q]))
-    with dt.Tracker.from_scene(scene) as trk:
-        for j in range(cfg.n_exp):
-            trk.load_image_batch(j, flux_pool[j % POOL:j % POOL + 1], var_pool[j % POOL:j % POOL + 1])
-        el = _elements_device(cfg, dev)
-        snr, hits = trk.stack(el, scene.t0)
-        st = trk.stats()
-        assert st["streamed"] == 1 and st["n_image_batches"] >= 2
-        assert st["h2d_image_bytes"] == cfg.image_bytes()
-        _whole_output_properties(dt, trk, snr, hits, cfg.n_exp)
-        sample = _pick_sample(scene, hits, cfg.n_orbits)
-        snr_h, hits_h = snr.cpu().numpy(), hits.cpu().numpy()
+    import os
+    el = _elements_device(cfg, dev)
+    results = {}
+    for mode in ("0", "-1"):      # streamed batch by batch, then the library's own choice (zero-copy gather)
+        os.environ["DT_STREAM_ZERO_COPY"] = mode
+        try:
+            with dt.Tracker.from_scene(scene) as trk:
+                for j in range(cfg.n_exp):
+                    trk.load_image_batch(j, flux_pool[j % POOL:j % POOL + 1], var_pool[j % POOL:j % POOL + 1])
+                snr, hits = trk.stack(el, scene.t0)
+                st = trk.stats()
+                assert st["streamed"] == 1 and st["n_image_batches"] >= 2
+                if mode == "0":
+                    assert st["image_zero_copy"] == 0 and st["h2d_image_bytes"] == cfg.image_bytes()
+                else:
+                    assert st["image_zero_copy"] == 1 and st["h2d_image_bytes"] == 0   # 6.8e4 hits: no image is copied
+                _whole_output_properties(dt, trk, snr, hits, cfg.n_exp)
+                results[mode] = (snr.cpu().numpy(), hits.cpu().numpy(), st)
+                if mode == "0":
+                    sample = _pick_sample(scene, hits, cfg.n_orbits)
+        finally:
+            os.environ.pop("DT_STREAM_ZERO_COPY", None)
+    assert np.array_equal(results["0"][0], results["-1"][0]) and np.array_equal(results["0"][1], results["-1"][1])
+    snr_h, hits_h, st = results["0"]
 
-        def plane_of(j):
-            return flux_pool[j % POOL].numpy(), var_pool[j % POOL].numpy()
+    def plane_of(j):
+        return flux_pool[j % POOL].numpy(), var_pool[j % POOL].numpy()
 
-        rep = _check_sample(cfg, scene, plane_of, snr_h, hits_h, sample, "lsst streamed")
-        gbs = st["h2d_image_bytes"] / (st["ms_total"] * 1e-3) * 1e-9
-        print("lsst streamed: pairs %.3g hits %d ms %.0f (%.1f GB/s host->device)" %
-              (cfg.pairs, st["hits"], st["ms_total"], gbs), rep)
+    rep = _check_sample(cfg, scene, plane_of, snr_h, hits_h, sample, "lsst streamed")
+    gbs = st["h2d_image_bytes"] / (st["ms_total"] * 1e-3) * 1e-9
+    print("lsst streamed: pairs %.3g hits %d ms %.0f (%.1f GB/s host->device); zero-copy gather: ms %.0f (%.3g pairs/s)" %
+          (cfg.pairs, st["hits"], st["ms_total"], gbs, results["-1"][2]["ms_total"],
+           cfg.pairs / (results["-1"][2]["ms_total"] * 1e-3)), rep)

@@ -223,9 +223,12 @@ def test_errors_and_state():
         dt.dt_create(sc.t, sc.obs_ecl, sc.ra0, sc.dec0, 0, 16, sc.pixel_scale, var_scalar=sc.var_scalar)
 
 
-def test_streaming_batches_match_resident():
+def test_streaming_batches_match_resident(monkeypatch):
     """north_star subsystem 4: a survey larger than the HBM budget is streamed from pinned host
-    memory in double-buffered exposure batches; results must equal the resident run bit for bit."""
+    memory in double-buffered exposure batches; results must equal the resident run bit for bit.
+    (The zero-copy gather, which would skip the copies on this short hit list, is switched off here
+    and tested in test_streaming_zero_copy_gather_matches_copied_batches.)"""
+    monkeypatch.setenv("DT_STREAM_ZERO_COPY", "0")
     dt = _dt()
     sc = _scene("lsst_focused")
     el = sc.elements()
@@ -434,3 +437,33 @@ def test_perihelion_stress_all_kepler_paths(flags):
         assert 0 < st["cold_solves"] < 0.5 * n * N, st          # and so was the cold solve, but rarely
     print("perihelion stress: flagged pixel mismatches %d, substep %d, cold %d of %d pairs" %
           (n_bad, st["substep_solves"], st["cold_solves"], n * N))
+
+
+@pytest.mark.parametrize("case,expect_auto", [("neo_diffuse", 1), ("tno_focused", None)])
+def test_streaming_zero_copy_gather_matches_copied_batches(case, expect_auto, monkeypatch):
+    """Streaming mode has two ways to reach the pixels: copy every exposure batch into the double
+    buffer, or -- when a probe predicts few hits -- gather straight from the page-locked host planes.
+    Forced copy, forced zero-copy and the library's own choice must agree bit for bit with each other
+    and with the resident run; the choice is zero-copy on a blind (diffuse) list."""
+    dt = _dt()
+    sc = _scene(case)
+    cfg = sc.cfg
+    el = sc.elements()
+    flux, var = _planes(sc, cfg.variance_mode)
+    with dt.Tracker.from_scene(sc) as trk:
+        trk.load_image_batch(0, flux, var)
+        snr_r, hits_r = trk.stack(el, sc.t0)
+    pf = torch.from_numpy(flux).pin_memory()
+    pv = torch.from_numpy(var).pin_memory() if var is not None else None
+    per_exp = flux[0].nbytes * (2 if var is not None else 1)
+    for mode, want in (("0", 0), ("1", 1), ("-1", expect_auto)):
+        monkeypatch.setenv("DT_STREAM_ZERO_COPY", mode)
+        with dt.Tracker.from_scene(sc, hbm_budget_bytes=2 * 20 * per_exp) as trk:
+            trk.load_image_batch(0, pf, pv)
+            snr_s, hits_s = trk.stack(el, sc.t0)
+            st = trk.stats()
+        assert st["streamed"] == 1
+        if want is not None:
+            assert st["image_zero_copy"] == want, (mode, st)
+        assert (st["h2d_image_bytes"] == 0) == (st["image_zero_copy"] == 1)
+        assert np.array_equal(hits_s, hits_r) and np.array_equal(snr_s, snr_r), mode
