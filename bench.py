@@ -314,15 +314,36 @@ def main():
     scene = ds.build_scene(cfg, project_fn)
     n = cfg.n_orbits
     el_np = rank_elements(cfg, rank, world)
-    trk = dt.Tracker.from_scene(scene, device=local_rank, flags=args.flags)
+    free_b, _total_b = torch.cuda.mem_get_info()
+    beyond_hbm = cfg.image_bytes() > 0.75 * free_b          # the library's own default budget
+    kw = {} if beyond_hbm else {"hbm_budget_bytes": cfg.image_bytes() + (1 << 30)}
+    trk = dt.Tracker.from_scene(scene, device=local_rank, flags=args.flags, **kw)
     trk_holder["t"] = trk
-    for j in range(cfg.n_exp):
-        f = scene.flux_plane_t(j, dev).unsqueeze(0).contiguous()
-        v = None
-        if cfg.variance_mode == 1:
-            v = torch.full((1, cfg.height, cfg.width), float(scene.var_scalar[j]), dtype=torch.float32,
-                           device=dev)
-        trk.load_image_batch(j, f, v)
+    keep_alive = []
+    if beyond_hbm:
+        # the survey does not fit HBM (configs[2]): page-locked host planes, streamed or gathered in place
+        # by the library.  The host holds a pool of distinct seeded exposures and exposure j registers
+        # pool[j mod POOL] (SURVEY.md 8(d) "Host memory"); pooled planes carry no injected sources.
+        POOL = 64
+        fpool = torch.empty((POOL, cfg.height, cfg.width), dtype=torch.float32).pin_memory()
+        vpool = torch.empty((POOL, cfg.height, cfg.width), dtype=torch.float32).pin_memory() \
+            if cfg.variance_mode == 1 else None
+        for q in range(POOL):
+            fpool[q].copy_(ds.noise_plane_t(cfg, q, dev))
+            if vpool is not None:
+                vpool[q].fill_(float(scene.var_scalar[q]))
+        for j in range(cfg.n_exp):
+            q = j % POOL
+            trk.load_image_batch(j, fpool[q:q + 1], vpool[q:q + 1] if vpool is not None else None)
+        keep_alive = [fpool, vpool]
+    else:
+        for j in range(cfg.n_exp):
+            f = scene.flux_plane_t(j, dev).unsqueeze(0).contiguous()
+            v = None
+            if cfg.variance_mode == 1:
+                v = torch.full((1, cfg.height, cfg.width), float(scene.var_scalar[j]), dtype=torch.float32,
+                               device=dev)
+            trk.load_image_batch(j, f, v)
     el_dev = torch.from_numpy(el_np).to(dev)
     el_pin = torch.from_numpy(el_np).pin_memory()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
@@ -417,7 +438,9 @@ def main():
                            "image": "%dx%d fp32" % (cfg.width, cfg.height),
                            "variance_mode": cfg.variance_mode, "flags": args.flags,
                            "parallelism": "replicas x%d" % world, "l2": "flushed between timed steps",
-                           "images_resident": not bool(stats["streamed"])},
+                           "images_resident": not bool(stats["streamed"]),
+                           "image_zero_copy": bool(stats["image_zero_copy"]),
+                           "h2d_image_bytes_per_step": int(stats["h2d_image_bytes"])},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(stats["launches"]) * args.steps,
                 "roofline": roofline,
                 "stages_ms": {"propagate": float(np.mean(ms_prop)), "gather": float(np.mean(ms_gath)),

@@ -130,7 +130,11 @@ int dt_destroy(dt_context *ctx);
  *     are COPIED into the context's image store in HBM and the caller may free them on return;
  *   - otherwise (streaming mode; north_star subsystem 4) the library RETAINS the pointers: they
  *     must be DT_MEM_PINNED (else DT_ERR_INVALID_ARG) and stay valid until dt_destroy or until the
- *     same exposure range is loaded again; dt_stack then streams them in double-buffered batches.
+ *     same exposure range is loaded again; dt_stack then streams them in double-buffered batches --
+ *     or, when a probe of the hit density predicts that the gathers would move less than 5 % of the
+ *     bytes streaming would (a blind search), copies no image and gathers the hit pixels straight
+ *     from the (device-mapped) page-locked planes; results are bit-identical either way
+ *     (dt_stats.image_zero_copy says which way was taken).
  * Ranges may be loaded in any order and re-loaded; overlapping a previously loaded range replaces it.
  */
 int dt_load_image_batch(dt_context *ctx, int32_t first_exposure, int32_t count, const float *flux,
