@@ -119,16 +119,21 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
 
             // ---- step 3: Kepler solve at t_j ----
             if (WARM) {
-                bool ok = false;
-                Kepler Kw = K;
-                if (have_state) Kw = kepler_warm<3>(o.e, K, M, ok);
-                if (__all_sync(0xffffffffu, ok)) {
-                    K = Kw;
-                } else {
-                    // some lane's step is too long for the narrow warm step (long gap, or close to
-                    // the perihelion of an eccentric orbit): take one wide warm step, or split the
-                    // step into equal wide sub-steps in M (count warp-uniform); only when that
-                    // would take too many, solve cold
+                // order 3 when every lane's step is short (main-belt cadences), else order 4, else --
+                // without spending the order-4 tail on a step that is outside its domain anyway --
+                // the wide paths
+                bool done = false;
+                if (have_state) {
+                    const WarmPre w = kepler_warm_pre(o.e, K, M);
+                    if (__all_sync(0xffffffffu, kepler_warm_in_domain<3>(w))) {
+                        K = kepler_warm_finish<3>(o.e, K, M, w);
+                        done = true;
+                    } else if (__all_sync(0xffffffffu, kepler_warm_in_domain<4>(w))) {
+                        K = kepler_warm_finish<4>(o.e, K, M, w);
+                        done = true;
+                    }
+                }
+                if (!done) {
                     bool solved = false;
                     if (have_state) {
                         const float r = __uint_as_float(
