@@ -324,21 +324,16 @@ __device__ __forceinline__ Kepler kepler_warm(double e, const Kepler &K0, double
 // Worst error of (u, sin E, cos E) against 40-digit solutions over 2e4 accepted random steps with
 // e <= 0.9: 6.5e-16 (the narrow step, with its single polish: 1.8e-13).
 // ~75 FP64 instructions against ~45 for the narrow step and several hundred for a cold solve.
-__device__ __forceinline__ Kepler kepler_warm_wide(double e, const Kepler &K0, double Mn, bool &ok)
+__device__ __forceinline__ Kepler kepler_warm_wide_finish(double e, const Kepler &K0, double Mn, const WarmPre &w,
+                                                          bool &ok)
 {
-    const double dM = Mn - K0.M;
-    const double es = e * K0.s, ec = e * K0.c;
-    const double f0 = (K0.u - es) - dM;
-    const double g = 1.0 - ec;
-    const double rg = rcp_nr<2>(g);
-    const double x = -f0 * rg;
-    const double a2 = 0.5 * es * rg;
-    const double a3 = (1.0 / 6.0) * ec * rg;
+    const double dM = w.dM, rg = w.rg, x = w.x, a2 = w.a2;
+    const double a3 = (1.0 / 6.0) * w.ec * rg;
     const double a22 = a2 * a2;
     const double k3 = fma(2.0, a22, -a3);
     const double k4 = fma(a2, fma(5.0, a3, 1.0 / 12.0), -5.0 * a22 * a2);
     const double th = x * fma(x, fma(x, fma(x, k4, k3), -a2), 1.0);
-    ok = (fabs(x) <= 0.3) && (fabs(x * a2) <= 0.08) && (fabs(a3) * x * x <= 0.02);
+    ok = (w.ax <= 0.3) && (w.axa2 <= 0.08) && (fabs(a3) * x * x <= 0.02);
     // Taylor rotation by th, sin to th^13, cos to th^12
     const double z = th * th;
     const double ps = fma(z, fma(z, fma(z, fma(z, fma(z, 1.0 / 6227020800.0, -1.0 / 39916800.0), 1.0 / 362880.0),
@@ -371,19 +366,18 @@ __device__ __forceinline__ Kepler kepler_warm_wide(double e, const Kepler &K0, d
     return K;
 }
 
-// How far outside kepler_warm_wide's accuracy domain a step toward Mn is: acceptable when the returned
-// ratio is <= 1 (its three tests; the quadratic one enters as a square root so that the ratio scales
-// like 1/ns under ns equal sub-steps).  A longer step is split by the caller into equal sub-steps in M, each a full wide warm step (series +
-// rotation + Newton polishes against its own directly computed M), which stays far cheaper than a
-// cold solve for several of them.
-__device__ __forceinline__ float kepler_warm_need(double e, const Kepler &K0, double Mn)
+__device__ __forceinline__ Kepler kepler_warm_wide(double e, const Kepler &K0, double Mn, bool &ok)
 {
-    const double dM = Mn - K0.M;
-    const double es = e * K0.s, ec = e * K0.c;
-    const double rg = rcp_nr<1>(1.0 - ec);
-    const double x = ((K0.u - es) - dM) * rg;
-    const float lin = (float)fmax(fabs(x) * (1.0 / 0.3), fabs(x * (0.5 * es * rg)) * (1.0 / 0.08));
-    const float cub = sqrtf((float)(fabs(ec * rg) * x * x * (1.0 / (6.0 * 0.02))));
+    return kepler_warm_wide_finish(e, K0, Mn, kepler_warm_pre(e, K0, Mn), ok);
+}
+
+// How far outside kepler_warm_wide's accuracy domain the step of prefix w is: acceptable when the
+// returned ratio is <= 1 (its three tests; the quadratic one enters as a square root so that the ratio
+// scales like 1/ns under ns equal sub-steps in M).
+__device__ __forceinline__ float kepler_warm_need_pre(const WarmPre &w)
+{
+    const float lin = (float)fmax(w.ax * (1.0 / 0.3), w.axa2 * (1.0 / 0.08));
+    const float cub = sqrtf((float)(fabs(w.ec * w.rg) * w.x * w.x * (1.0 / (6.0 * 0.02))));
     return fmaxf(lin, cub);
 }
 

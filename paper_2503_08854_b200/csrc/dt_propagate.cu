@@ -122,33 +122,36 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 // order 3 when every lane's step is short (main-belt cadences), else order 4, else --
                 // without spending the order-4 tail on a step that is outside its domain anyway --
                 // the wide paths
-                bool done = false;
+                bool solved = false;
                 if (have_state) {
                     const WarmPre w = kepler_warm_pre(o.e, K, M);
                     if (__all_sync(0xffffffffu, kepler_warm_in_domain<3>(w))) {
                         K = kepler_warm_finish<3>(o.e, K, M, w);
-                        done = true;
+                        solved = true;
                     } else if (__all_sync(0xffffffffu, kepler_warm_in_domain<4>(w))) {
                         K = kepler_warm_finish<4>(o.e, K, M, w);
-                        done = true;
-                    }
-                }
-                if (!done) {
-                    bool solved = false;
-                    if (have_state) {
+                        solved = true;
+                    } else {
+                        // some lane's step is too long (a long gap, or close to the perihelion of an
+                        // eccentric orbit): one wide warm step from the same prefix, or equal wide
+                        // sub-steps in M (count warp-uniform).  r <= 1 is the wide step's own domain;
+                        // the margins leave room for the coefficients growing on the way to a
+                        // perihelion (every step re-checks its domain)
                         const float r = __uint_as_float(
-                            __reduce_max_sync(0xffffffffu, __float_as_uint(kepler_warm_need(o.e, K, M))));
-                        // r <= 1 is the wide step's own domain; the margins leave room for the
-                        // coefficients growing on the way to a perihelion (every sub-step re-checks)
+                            __reduce_max_sync(0xffffffffu, __float_as_uint(kepler_warm_need_pre(w))));
                         if (r < (float)kMaxSubsteps / 1.3f) {       // false for NaN
                             const int ns = (r <= 0.8f) ? 1 : (int)ceilf(1.3f * r);
-                            const double M_from = K.M, dMs = (M - M_from) / (double)ns;
                             Kepler Kc = K;
                             bool good = true;
-                            for (int sidx = 1; sidx <= ns; ++sidx) {
-                                bool oks;
-                                Kc = kepler_warm_wide(o.e, Kc, (sidx == ns) ? M : fma(dMs, (double)sidx, M_from), oks);
-                                good = good && oks;
+                            if (ns == 1) {
+                                Kc = kepler_warm_wide_finish(o.e, K, M, w, good);
+                            } else {
+                                const double M_from = K.M, dMs = (M - M_from) / (double)ns;
+                                for (int sidx = 1; sidx <= ns; ++sidx) {
+                                    bool oks;
+                                    Kc = kepler_warm_wide(o.e, Kc, (sidx == ns) ? M : fma(dMs, (double)sidx, M_from), oks);
+                                    good = good && oks;
+                                }
                             }
                             if (__all_sync(0xffffffffu, good)) {
                                 K = Kc;
@@ -157,10 +160,10 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                             }
                         }
                     }
-                    if (!solved) {
-                        K = kepler_cold(o.e, M);
-                        n_cold += 1;
-                    }
+                }
+                if (!solved) {
+                    K = kepler_cold(o.e, M);
+                    n_cold += 1;
                 }
                 have_state = true;
             } else {
