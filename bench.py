@@ -38,8 +38,8 @@ UNIT = "pairs/s"
 FP64_SLOTS_COARSE = 66.0     # order-3 warm Kepler step + geometric position + cone test (every pair)
 FP64_SLOTS_REFINE = 70.0     # light-time re-solve + projection + footprint test (refined pairs only)
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_propagate<3> launch on configs[1], from the
-# `ncu --set full` capture summarised in profiles/r1c_final.md (48.11 MB + 19.42 MB)
-K1_TRAFFIC_BYTES_SMALL_MBA = 67.54e6
+# `ncu --set full` capture summarised in profiles/r1c_final.md (48.18 MB + 19.01 MB)
+K1_TRAFFIC_BYTES_SMALL_MBA = 67.19e6
 
 
 def parse_args():
