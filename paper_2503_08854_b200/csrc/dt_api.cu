@@ -47,7 +47,8 @@ struct dt_context {
     // image store
     bool streaming = false;
     int64_t budget = 0;
-    float *d_flux = nullptr, *d_var = nullptr;          // resident: N planes each
+    float *d_flux = nullptr, *d_var = nullptr;          // resident: N planes each (scalar-variance mode: flux only)
+    float2 *d_fv = nullptr;                             // resident, plane-variance mode: (flux, var) interleaved per pixel
     std::vector<uint8_t> loaded;                        // per exposure
     std::vector<const float *> h_flux, h_var;           // streaming: retained pinned pointers
     float *d_buf_flux[2] = {nullptr, nullptr}, *d_buf_var[2] = {nullptr, nullptr};
@@ -122,6 +123,7 @@ void free_all(dt_context *c)
     cudaFree(c->d_exp);
     cudaFree(c->d_flux);
     cudaFree(c->d_var);
+    cudaFree(c->d_fv);
     for (int s = 0; s < 2; ++s) {
         cudaFree(c->d_buf_flux[s]);
         cudaFree(c->d_buf_var[s]);
@@ -209,8 +211,11 @@ int ensure_store(dt_context *c)
         }
         return DT_OK;
     }
-    if (!c->d_flux) CU(c, cudaMalloc((void **)&c->d_flux, (size_t)(c->N * c->plane) * 4));
-    if (c->var_mode == 1 && !c->d_var) CU(c, cudaMalloc((void **)&c->d_var, (size_t)(c->N * c->plane) * 4));
+    if (c->var_mode == 1) {
+        if (!c->d_fv) CU(c, cudaMalloc((void **)&c->d_fv, (size_t)(c->N * c->plane) * 8));
+    } else if (!c->d_flux) {
+        CU(c, cudaMalloc((void **)&c->d_flux, (size_t)(c->N * c->plane) * 4));
+    }
     return DT_OK;
 }
 
@@ -340,10 +345,38 @@ int dt_load_image_batch(dt_context *c, int32_t first, int32_t count, const float
     }
     int rc = ensure_store(c);
     if (rc != DT_OK) return rc;
-    const size_t bytes = (size_t)count * (size_t)c->plane * 4;
-    CU(c, cudaMemcpyAsync(c->d_flux + (int64_t)first * c->plane, flux, bytes, cudaMemcpyDefault, c->stream));
-    if (c->var_mode == 1)
-        CU(c, cudaMemcpyAsync(c->d_var + (int64_t)first * c->plane, var, bytes, cudaMemcpyDefault, c->stream));
+    if (c->var_mode == 1) {
+        // plane-variance mode: the store interleaves (flux, var) per pixel.  Device sources are read in
+        // place; host sources go through a staging buffer a few planes at a time.
+        float2 *dst = c->d_fv + (int64_t)first * c->plane;
+        if (mem_kind == DT_MEM_DEVICE) {
+            CU(c, launch_interleave(flux, var, dst, (int64_t)count * c->plane, c->stream));
+        } else {
+            const int32_t chunk = std::min<int32_t>(count, 4);
+            float *stage = nullptr;
+            CU(c, cudaMalloc((void **)&stage, (size_t)chunk * (size_t)c->plane * 8));
+            for (int32_t j = 0; j < count; j += chunk) {
+                const int32_t m = std::min<int32_t>(chunk, count - j);
+                const size_t b = (size_t)m * (size_t)c->plane * 4;
+                cudaError_t e = cudaMemcpyAsync(stage, flux + (int64_t)j * c->plane, b, cudaMemcpyHostToDevice, c->stream);
+                if (e == cudaSuccess)
+                    e = cudaMemcpyAsync(stage + (int64_t)chunk * c->plane, var + (int64_t)j * c->plane, b,
+                                        cudaMemcpyHostToDevice, c->stream);
+                if (e == cudaSuccess)
+                    e = launch_interleave(stage, stage + (int64_t)chunk * c->plane, dst + (int64_t)j * c->plane,
+                                          (int64_t)m * c->plane, c->stream);
+                if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+                if (e != cudaSuccess) {
+                    cudaFree(stage);
+                    return fail(c, DT_ERR_CUDA, "dt_load_image_batch: %s", cudaGetErrorString(e));
+                }
+            }
+            cudaFree(stage);
+        }
+    } else {
+        const size_t bytes = (size_t)count * (size_t)c->plane * 4;
+        CU(c, cudaMemcpyAsync(c->d_flux + (int64_t)first * c->plane, flux, bytes, cudaMemcpyDefault, c->stream));
+    }
     CU(c, cudaStreamSynchronize(c->stream));
     for (int32_t j = 0; j < count; ++j) c->loaded[first + j] = 1;
     return DT_OK;
@@ -599,8 +632,8 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
                 g.flux = c->d_buf_flux[slot] - (int64_t)first * c->plane;
                 g.var = (c->var_mode == 1) ? c->d_buf_var[slot] - (int64_t)first * c->plane : nullptr;
             } else {
-                g.flux = c->d_flux;
-                g.var = (c->var_mode == 1) ? c->d_var : nullptr;
+                g.flux = c->d_flux;              // scalar-variance mode
+                g.fv = c->d_fv;                  // plane-variance mode (one of the two is NULL)
             }
             g.exp_all = c->d_exp;
             g.plane = c->plane;
@@ -736,7 +769,7 @@ int dt_gather_hits(dt_context *c, int64_t n, int32_t first_exposure, int32_t n_g
     if (n > kMaxUnitOrbits || n_groups > kMaxUnitExposures / kGroup)
         return fail(c, DT_ERR_INVALID_ARG, "dt_gather_hits: at most %lld orbits and %d groups per call",
                     (long long)kMaxUnitOrbits, kMaxUnitExposures / kGroup);
-    if (c->streaming || !c->d_flux) return fail(c, DT_ERR_STATE, "dt_gather_hits needs resident images");
+    if (c->streaming || (!c->d_flux && !c->d_fv)) return fail(c, DT_ERR_STATE, "dt_gather_hits needs resident images");
     CU(c, cudaSetDevice(c->device));
     GatherParams g;
     memset(&g, 0, sizeof g);
@@ -748,7 +781,7 @@ int dt_gather_hits(dt_context *c, int64_t n, int32_t first_exposure, int32_t n_g
     g.base = (const unsigned long long *)base;
     g.offsets = offsets;
     g.flux = c->d_flux;
-    g.var = (c->var_mode == 1) ? c->d_var : nullptr;
+    g.fv = c->d_fv;
     g.exp_all = c->d_exp;
     g.plane = c->plane;
     g.S = S;

@@ -69,6 +69,10 @@ struct GatherParams {
     const uint32_t *offsets;
     const float *flux;          // plane of ABSOLUTE exposure j at flux + j * plane
     const float *var;           // same indexing; NULL in scalar mode
+    // resident plane-variance store: flux and variance INTERLEAVED per pixel, (flux, var) of absolute
+    // exposure j, pixel off at fv[j * plane + off]: one 8-B gather per hit instead of two 4-B gathers
+    // into different planes (gathers are bound by the access rate, not by bytes); flux / var NULL then
+    const float2 *fv;
     // zero-copy mode (sparse schedule only): per-exposure plane pointers, absolute index, device-mapped
     // page-locked HOST memory; flux / var above are NULL then
     const float *const *flux_ptrs;
@@ -96,6 +100,8 @@ constexpr int kGatherCtasPerSm = 1024 / kGatherThreads;   // 1024 resident threa
 constexpr int kMaxTilesPerWarp = 8;     // 148 SMs x 32 warps x 8 tiles x 32 orbits >= 2^20 orbits
 
 cudaError_t launch_gather(const GatherParams &p, int device, cudaStream_t stream);
+// dst[k] = (flux[k], var[k]), k < n: builds the interleaved store from two device planes
+cudaError_t launch_interleave(const float *flux, const float *var, float2 *dst, int64_t n, cudaStream_t stream);
 
 // SNR finalisation: snr = S / sqrt(Wt) (0 when no hit), NaN / -1 for invalid orbits.
 cudaError_t launch_finalize(const double *elements, int64_t n, const double *S, const double *Wt,

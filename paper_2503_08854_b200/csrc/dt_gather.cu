@@ -21,6 +21,8 @@
 // Both accumulate S += f/v, Wt += 1/v per orbit in ascending exposure order in a lane-private
 // accumulator (registers here, shared memory in the dense kernel) -- no atomics, and bit-identical
 // to a sequential evaluation of the definition.
+#include <algorithm>
+
 #include "dt_common.cuh"
 #include "dt_gather.cuh"
 
@@ -96,6 +98,10 @@ __global__ void __launch_bounds__(kSparseThreads) k_gather_sparse(const GatherPa
                         // zero-copy: the pixel comes straight from page-locked host memory over PCIe
                         f[q] = ld_pixel_cached(p.flux_ptrs[j0 + jj[q]] + off[q]);
                         if (PLANE_VAR) vv[q] = ld_pixel_cached(p.var_ptrs[j0 + jj[q]] + off[q]);
+                    } else if (PLANE_VAR && p.fv) {
+                        const float2 t2 = ld_pixel2_cached(p.fv + ((j0 + jj[q]) * p.plane + off[q]));
+                        f[q] = t2.x;
+                        vv[q] = t2.y;
                     } else {
                         const int64_t a = (j0 + jj[q]) * p.plane + off[q];
                         if (cached) {
@@ -139,7 +145,7 @@ cudaError_t launch_gather(const GatherParams &p_in, int device, cudaStream_t str
     if (p.window < 1) p.window = 1;
     if (p.lockstep_mode != 1) {
         const unsigned blocks = (unsigned)((p.n_pad + kSparseThreads - 1) / kSparseThreads);
-        if (p.var || p.var_ptrs)
+        if (p.var || p.var_ptrs || p.fv)
             k_gather_sparse<true><<<blocks, kSparseThreads, 0, stream>>>(p);
         else
             k_gather_sparse<false><<<blocks, kSparseThreads, 0, stream>>>(p);
@@ -148,6 +154,22 @@ cudaError_t launch_gather(const GatherParams &p_in, int device, cudaStream_t str
     }
     if (p.lockstep_mode != 0) return launch_gather_dense(p, device, stream);
     return cudaSuccess;
+}
+
+// ---- interleaved store ------------------------------------------------------------------------------------
+__global__ void k_interleave(const float *__restrict__ flux, const float *__restrict__ var, float2 *__restrict__ dst,
+                             int64_t n)
+{
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x)
+        dst[k] = make_float2(flux[k], var[k]);
+}
+
+cudaError_t launch_interleave(const float *flux, const float *var, float2 *dst, int64_t n, cudaStream_t stream)
+{
+    if (n <= 0) return cudaSuccess;
+    const unsigned blocks = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
+    k_interleave<<<blocks, 256, 0, stream>>>(flux, var, dst, n);
+    return cudaGetLastError();
 }
 
 // ---- finalisation ---------------------------------------------------------------------------------------

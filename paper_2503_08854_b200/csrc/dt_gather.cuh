@@ -23,6 +23,14 @@ __device__ __forceinline__ float ld_pixel_cached(const float *p)
     return v;
 }
 
+// (flux, variance) of one pixel of the interleaved store
+__device__ __forceinline__ float2 ld_pixel2_cached(const float2 *p)
+{
+    float2 v;
+    asm volatile("ld.global.nc.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
+
 // Steps 9-10 for one hit: skipped (not counted) unless f, v finite and v > 0; w = 1/v.
 __device__ __forceinline__ void stack_one(double f, double v, double w, double &S, double &Wt, int32_t &cnt)
 {

@@ -136,7 +136,11 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherCtasPerSm) k_gather_den
                 f[t] = 0.f;
                 vv[t] = 1.f;
                 if ((mine >> t) & 1u) {
-                    if (cached) {
+                    if (PLANE_VAR && p.fv) {
+                        const float2 t2 = ld_pixel2_cached(p.fv + ((j0 + jj) * p.plane + off[t]));
+                        f[t] = t2.x;
+                        vv[t] = t2.y;
+                    } else if (cached) {
                         f[t] = ld_pixel_cached(fplane + off[t]);
                         if (PLANE_VAR) vv[t] = ld_pixel_cached(vplane + off[t]);
                     } else {
@@ -232,9 +236,10 @@ cudaError_t launch_gather_dense(const GatherParams &p_in, int device, cudaStream
     p.tiles_per_warp = T;
     e = cudaMemsetAsync(p.progress, 0, (size_t)p.n_groups * kGroup * kProgressStride * sizeof(int), stream);
     if (e != cudaSuccess) return e;
-    const void *fn = p.var ? (const void *)k_gather_dense<true> : (const void *)k_gather_dense<false>;
+    const bool plane_var = p.var || p.fv;
+    const void *fn = plane_var ? (const void *)k_gather_dense<true> : (const void *)k_gather_dense<false>;
     static size_t smem_set[2] = {0, 0};
-    const int which = p.var ? 1 : 0;
+    const int which = plane_var ? 1 : 0;
     if (smem > smem_set[which]) {
         e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
