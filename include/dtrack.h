@@ -144,7 +144,11 @@ int dt_load_image_batch(dt_context *ctx, int32_t first_exposure, int32_t count, 
  * dt_stack: the hot path (steps 1-8 above) for n orbits against all exposures.
  *   elements  [n][6] = a (AU), e, i, Omega, omega, M0 (rad), fp64, in memory `mem_kind`
  *   t0        epoch of M0, days (one per call)
- *   snr_out   [n] fp64, hits_out [n] int32, in memory `mem_kind` (either may be NULL)
+ *   snr_out   [n] fp64, hits_out [n] int32 (either may be NULL): device memory when mem_kind is
+ *             DT_MEM_DEVICE, else host memory (pageable or page-locked; page-locked is faster)
+ * DT_MEM_PINNED elements (16-byte aligned) are not copied to the device first: kernel 1 reads each
+ * tile of 128 orbits with one bulk copy straight from the page-locked buffer while earlier tiles
+ * compute, so the buffer must stay valid (and unchanged) until the call returns.
  * Invalid orbits do not fail the call: they get hits = -1, snr = NaN.  Results are complete when
  * the call returns (the call synchronises the context stream).  The per-orbit results also stay
  * on the device for dt_topk.  Errors: DT_ERR_NOT_LOADED unless every exposure has images.
