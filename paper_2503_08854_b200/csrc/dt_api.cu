@@ -71,6 +71,7 @@ struct dt_context {
     int32_t gather_window = 1;                          // exposures the slowest and fastest CTA may be apart
     int32_t gather_lockstep = -1;                       // -1: decided on the device from the hit density
     int32_t gather_ld_cached = 1;
+    int32_t gather_prefetch = 1;                        // DT_GATHER_PREFETCH: planes ahead (dense schedule, resident store)
     int32_t stream_zero_copy = -1;                      // DT_STREAM_ZERO_COPY: -1 decide from a probe, 0 never, 1 always
     const float **d_flux_ptrs = nullptr, **d_var_ptrs = nullptr;   // [N] device-mapped pinned planes (zero-copy gather)
     bool zero_copy_elements = true;                     // DT_ZERO_COPY=0: copy pinned elements to the device first
@@ -289,6 +290,7 @@ int dt_create(const dt_survey *s, dt_context **out)
         c->gather_window = pick_gather_window(c);
         if (const char *env = getenv("DT_STREAM_ZERO_COPY")) c->stream_zero_copy = atoi(env) < 0 ? -1 : (atoi(env) ? 1 : 0);
         if (const char *env = getenv("DT_ZERO_COPY")) c->zero_copy_elements = atoi(env) != 0;
+        if (const char *env = getenv("DT_GATHER_PREFETCH")) c->gather_prefetch = std::max(0, std::min(atoi(env), 8));
         if (const char *env = getenv("DT_GATHER_L1")) c->gather_ld_cached = atoi(env) ? 1 : 0;
         if (const char *env = getenv("DT_GATHER_LOCKSTEP")) c->gather_lockstep = atoi(env) < 0 ? -1 : (atoi(env) ? 1 : 0);
         if (cudaStreamSynchronize(c->stream) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
@@ -645,6 +647,8 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
             g.n_hits_dev = c->d_counters;            // the unit's hit allocator, final after kernel 1
             g.lockstep_mode = zero_copy_images ? 0 : c->gather_lockstep;
             g.ld_cached = c->gather_ld_cached;
+            g.prefetch = c->streaming ? 0 : c->gather_prefetch;
+            g.n_exp_store = c->N;
             CU(c, launch_gather(g, c->device, c->stream));
             st.gather_launches += (g.lockstep_mode < 0) ? 2 : 1;   // sparse + dense schedule, one of them returns at once
             CU(c, cudaEventRecord(ev_at(3 * unit_idx + 2), c->stream));
@@ -793,6 +797,8 @@ int dt_gather_hits(dt_context *c, int64_t n, int32_t first_exposure, int32_t n_g
     g.n_hits_host = n_hits;
     g.lockstep_mode = c->gather_lockstep;
     g.ld_cached = c->gather_ld_cached;
+    g.prefetch = c->gather_prefetch;
+    g.n_exp_store = c->N;
     CU(c, launch_gather(g, c->device, c->stream));
     return DT_OK;
 }

@@ -88,6 +88,8 @@ struct GatherParams {
     int64_t n_hits_host;        // used when n_hits_dev is NULL
     int32_t lockstep_mode;      // -1: decide from the hit density; 0: sparse schedule; 1: dense schedule
     int32_t ld_cached;          // dense schedule: pixel loads allocate in L1 (1) or not (0)
+    int32_t prefetch;           // dense schedule: planes ahead of the front that are prefetched into L2 (0 = off)
+    int32_t n_exp_store;        // exposures the store holds from absolute index 0 (bound of the prefetch)
 };
 
 constexpr int kProgressStride = 32;     // one 128-B line per exposure counter (no false sharing of polls)

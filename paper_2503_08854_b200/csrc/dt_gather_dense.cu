@@ -29,6 +29,10 @@ __device__ __forceinline__ int ld_relaxed(const int *p)
     asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+__device__ __forceinline__ void prefetch_l2(const void *p)
+{
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
 __device__ __forceinline__ void red_add_relaxed(int *p, int v)
 {
     asm volatile("red.relaxed.gpu.global.add.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
@@ -62,6 +66,7 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherCtasPerSm) k_gather_den
 
     // tiles this warp owns: gw + t NW, t < T (bit t of `owned`); this lane's orbit in tile t
     uint32_t owned = 0, touched = 0;
+    bool spread = false;      // this warp's hits of the last exposure spanned more than half the plane
 #pragma unroll
     for (int t = 0; t < kMaxTilesPerWarp; ++t)
         if (t < T && gw + (int64_t)t * NW < n_tiles) owned |= 1u << t;
@@ -117,6 +122,22 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherCtasPerSm) k_gather_den
                     }
                 }
             }
+            // ---- L2 prefetch of the next plane, when this warp's hits are spread over the plane ----
+            // About half of the gathers of a uniformly hit plane are first touches of their line: DRAM
+            // latency, and DRAM accessed line by line in gather order.  If the warp's hits of the
+            // previous exposure spanned more than half the plane, every thread prefetches its share
+            // (<= one 128-B line per thread and exposure) of the plane `prefetch` exposures ahead, which
+            // then enters L2 as a sequential stream.  Clustered hit lists do not trigger it (a
+            // whole-plane prefetch would waste DRAM bandwidth there).
+            if (spread && p.first_exposure + jl + p.prefetch < p.n_exp_store) {
+                const int64_t n_lines = (p.plane * (PLANE_VAR && p.fv ? 8 : 4) + 127) >> 7;
+                const char *base = PLANE_VAR && p.fv
+                                       ? reinterpret_cast<const char *>(p.fv + (j0 + jj + p.prefetch) * p.plane)
+                                       : reinterpret_cast<const char *>(p.flux + (j0 + jj + p.prefetch) * p.plane);
+                for (int64_t l = (int64_t)blockIdx.x * kGatherThreads + threadIdx.x; l < n_lines;
+                     l += (int64_t)gridDim.x * kGatherThreads)
+                    prefetch_l2(base + l * 128);
+            }
             // ---- locate this lane's entry in each tile's block, read offsets (coalesced) ----
             uint32_t off[kMaxTilesPerWarp];
             uint32_t mine = 0;
@@ -127,6 +148,20 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherCtasPerSm) k_gather_den
                 off[t] = h ? p.offsets[cur[t] + __popc(hm & lt)] : 0u;
                 cur[t] += __popc(hm);
                 mine |= h ? (1u << t) : 0u;
+            }
+            // ---- is this warp's hit set spread over the plane?  (predictor for the prefetch below) ----
+            if (p.prefetch > 0) {
+                uint32_t omin = 0xffffffffu, omax = 0u;
+#pragma unroll
+                for (int t = 0; t < kMaxTilesPerWarp; ++t) {
+                    if ((mine >> t) & 1u) {
+                        omin = min(omin, off[t]);
+                        omax = max(omax, off[t]);
+                    }
+                }
+                omin = __reduce_min_sync(0xffffffffu, omin);
+                omax = __reduce_max_sync(0xffffffffu, omax);
+                spread = omax > omin && (int64_t)(omax - omin) * 2 > p.plane;
             }
             const float *fplane = p.flux + (j0 + jj) * p.plane;
             const float *vplane = PLANE_VAR ? p.var + (j0 + jj) * p.plane : nullptr;
