@@ -296,8 +296,13 @@ def test_more_than_one_orbit_unit():
     print(rep)
 
 
-def test_gather_hits_entry_matches_definition():
-    """dt_gather_hits on a hand-built hit list: every pair hits a seeded random pixel."""
+@pytest.mark.parametrize("schedule", ["auto", "sparse", "dense"])
+def test_gather_hits_entry_matches_definition(schedule, monkeypatch):
+    """dt_gather_hits on a hand-built hit list: every pair hits a seeded random pixel.  Both schedules of
+    kernel 3 (forced through DT_GATHER_LOCKSTEP) and the library's own choice must give exactly the
+    sequential sums of the definition."""
+    if schedule != "auto":
+        monkeypatch.setenv("DT_GATHER_LOCKSTEP", "1" if schedule == "dense" else "0")
     dt = _dt()
     N, H, W, n = 64, 96, 80, 1000
     rng = np.random.default_rng(5)
