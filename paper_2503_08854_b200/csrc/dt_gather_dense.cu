@@ -104,6 +104,7 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherCtasPerSm) k_gather_den
         }
 
         const int64_t j0 = (int64_t)p.first_exposure + (int64_t)g * kGroup;
+        bool check_spread = true;
         while (gm) {
             const int jj = __ffs(gm) - 1;
             gm &= gm - 1;
@@ -149,8 +150,10 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherCtasPerSm) k_gather_den
                 cur[t] += __popc(hm);
                 mine |= h ? (1u << t) : 0u;
             }
-            // ---- is this warp's hit set spread over the plane?  (predictor for the prefetch below) ----
-            if (p.prefetch > 0) {
+            // ---- is this warp's hit set spread over the plane?  (predictor for the prefetch above;
+            // re-evaluated on the first exposure of every group only: the reuse regime is issue-bound) ----
+            if (p.prefetch > 0 && check_spread) {
+                check_spread = false;
                 uint32_t omin = 0xffffffffu, omax = 0u;
 #pragma unroll
                 for (int t = 0; t < kMaxTilesPerWarp; ++t) {
