@@ -214,7 +214,28 @@ __device__ __forceinline__ Kepler kepler_newton_from(double e, const Kepler &K0,
 //                                                               FP64 instructions
 //   ORDER 2: |x| <= 0.003, |x a2| <= 0.001   (worst 5.9e-16)   the light-time re-solve (x ~ n tau):
 //                                                               13 fewer
-template <int ORDER>
+// One Newton step on the carried state: f = u - e s, 1/g from its own MUFU seed + one Newton step
+// (1e-12 relative, measured).  One Newton step from the previous 1/g instead leaves ((g1 - g)/g)^2 of
+// the correction behind, up to 1.3e-10 rad at e = 0.9 next to a perihelion.
+__device__ __forceinline__ Kepler kepler_polish(double e, const Kepler &K0)
+{
+    const double f1 = fma(-e, K0.s, K0.u);
+    const double g1 = fma(-e, K0.c, 1.0);
+    const double d = -f1 * rcp_nr<1>(g1);
+    Kepler K;
+    K.M = K0.M;
+    K.u = K0.u + d;
+    K.s = fma(d, K0.c, K0.s);
+    K.c = fma(-d, K0.s, K0.c);
+    return K;
+}
+
+// POLISH = false returns the state right after the series step and the rotation: a self-consistent
+// point (s = sin(M + u), c = cos(M + u)) whose u is off by the series truncation (<= 6.5e-8 rad for
+// ORDER 3, chained steps included: the next step's series starts from the exact residual of the
+// state it is given, so the error does not accumulate).  Good enough to CULL with; kepler_polish
+// finishes the job for the pairs that survive.
+template <int ORDER, bool POLISH = true>
 __device__ __forceinline__ Kepler kepler_warm_tail(double e, const Kepler &K0, double Mn, double dM, double es,
                                                    double ec, double rg, double x, double a2)
 {
@@ -252,19 +273,12 @@ __device__ __forceinline__ Kepler kepler_warm_tail(double e, const Kepler &K0, d
     const double s1 = fma(K0.s, cm, fma(K0.c, st, K0.s));
     const double c1 = fma(K0.c, cm, fma(-K0.s, st, K0.c));
     const double u1 = K0.u + (th - dM);
-    // Newton polish: f1 = u1 - e s1, and 1/g1 from its own MUFU seed + one Newton step (1e-12
-    // relative, measured; d <= ~1e-6).  One Newton step from rg instead leaves ((g1 - g)/g)^2 of d,
-    // up to 1.3e-10 rad at e = 0.9 next to a perihelion.
-    const double f1 = fma(-e, s1, u1);
-    const double g1 = fma(-e, c1, 1.0);
-    const double rg1 = rcp_nr<1>(g1);
-    const double d = -f1 * rg1;
     Kepler K;
     K.M = Mn;
-    K.u = u1 + d;
-    K.s = fma(d, c1, s1);
-    K.c = fma(-d, s1, c1);
-    return K;
+    K.u = u1;
+    K.s = s1;
+    K.c = c1;
+    return POLISH ? kepler_polish(e, K) : K;
 }
 
 // The part of the warm step that comes before its order is known: first-order step x and a2.
@@ -293,10 +307,10 @@ __device__ __forceinline__ bool kepler_warm_in_domain(const WarmPre &w)
     if (ORDER == 3) return (w.ax <= C[11]) && (w.axa2 <= C[12]);
     return (w.ax <= C[13]) && (w.axa2 <= C[14]);
 }
-template <int ORDER>
+template <int ORDER, bool POLISH = true>
 __device__ __forceinline__ Kepler kepler_warm_finish(double e, const Kepler &K0, double Mn, const WarmPre &w)
 {
-    return kepler_warm_tail<ORDER>(e, K0, Mn, w.dM, w.es, w.ec, w.rg, w.x, w.a2);
+    return kepler_warm_tail<ORDER, POLISH>(e, K0, Mn, w.dM, w.es, w.ec, w.rg, w.x, w.a2);
 }
 
 // LOW = 3 for the exposure-to-exposure step, 2 for the light-time re-solve: the warp takes the cheaper

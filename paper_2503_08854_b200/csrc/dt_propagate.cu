@@ -99,6 +99,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
     K.M = K.u = K.s = 0.0;
     K.c = 1.0;
     bool have_state = false;
+    bool prev_refined = false;     // warp-uniform: the last exposure's pairs went through the refinement
     unsigned long long n_refined = 0, n_cold = 0, n_hits = 0, n_sub = 0;
 
     for (int g = g_begin; g < g_end; ++g) {
@@ -118,15 +119,27 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
             const double M = fma(o.n, dt, o.M0);
 
             // ---- step 3: Kepler solve at t_j ----
+            bool unpolished = false;       // warp-uniform: K still lacks its Newton polish
             if (WARM) {
                 // order 3 when every lane's step is short (main-belt cadences), else order 4, else --
                 // without spending the order-4 tail on a step that is outside its domain anyway --
                 // the wide paths
                 bool solved = false;
+                unpolished = false;
                 if (have_state) {
                     const WarmPre w = kepler_warm_pre(o.e, K, M);
                     if (__all_sync(0xffffffffu, kepler_warm_in_domain<3>(w))) {
-                        K = kepler_warm_finish<3>(o.e, K, M, w);
+                        // with the pre-cull the Newton polish is deferred to the pairs that survive it:
+                        // the unpolished state is off by <= 6.5e-8 rad in E, far inside the cone's slack
+                        // (objects closer than 0.1 AU are always refined, see `near` below)
+                        // (a warp whose last pair survived the cull -- a focused search -- polishes at
+                        // once: deferring would cost it the geometric distance twice)
+                        if (PRECULL && !prev_refined) {
+                            K = kepler_warm_finish<3, false>(o.e, K, M, w);
+                            unpolished = true;
+                        } else {
+                            K = kepler_warm_finish<3, true>(o.e, K, M, w);
+                        }
                         solved = true;
                     } else if (__all_sync(0xffffffffu, kepler_warm_in_domain<4>(w))) {
                         K = kepler_warm_finish<4>(o.e, K, M, w);
@@ -183,14 +196,28 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 // conservative cone test on the GEOMETRIC direction (see orbit_setup)
                 const double D0 = fma(dx0, x.tx, fma(dy0, x.ty, dz0 * x.tz));
                 near = !(D0 * D0 < o.cos2_cull * rho2) && (D0 > 0.0 || o.cos2_cull < 0.0);
-                near = near || !(rho2 > 1e-12);
+                // always refine objects closer than 0.1 AU: there a state error of 6.5e-8 rad in E could
+                // move the direction by more than the cone's 2e-5 rad slack (and rho2 ~ 0 must not cull)
+                near = near || !(rho2 > 0.01);
             }
             bool hit = false;
             int32_t ix = -1, iy = -1;
             double xpix = 0.0, ypix = 0.0, qx = 0.0, qy = 0.0, qz = 0.0;
-            if (!PRECULL || __any_sync(0xffffffffu, near)) {
+            const bool refine = !PRECULL || __any_sync(0xffffffffu, near);
+            prev_refined = refine;
+            if (refine) {
                 n_refined += 1;
-                const double rho0 = WARM ? sqrt_nr<2>(rho2) : sqrt(rho2);
+                double rho2r = rho2;
+                if (unpolished) {
+                    // the deferred polish, then the geometric distance again from the polished state
+                    K = kepler_polish(o.e, K);
+                    const double X0p = K.c - o.e;
+                    const double ax0 = fma(o.Ax, X0p, fma(o.Bx, K.s, -x.Rx));
+                    const double ay0 = fma(o.Ay, X0p, fma(o.By, K.s, -x.Ry));
+                    const double az0 = fma(o.Az, X0p, fma(o.Bz, K.s, -x.Rz));
+                    rho2r = fma(ax0, ax0, fma(ay0, ay0, az0 * az0));
+                }
+                const double rho0 = WARM ? sqrt_nr<2>(rho2r) : sqrt(rho2r);
                 const double tau = rho0 * p.inv_c;
                 const double M1 = fma(o.n, dt - tau, o.M0);
                 Kepler K1;
