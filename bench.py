@@ -42,8 +42,8 @@ UNIT = "pairs/s"
 FP64_SLOTS_COARSE = 58.25    # every pair
 FP64_SLOTS_REFINE = 78.0     # refined pairs only, on top
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_propagate<3> launch on configs[1], from the
-# `ncu --set full` capture summarised in profiles/r1c_final.md (48.18 MB + 19.01 MB)
-K1_TRAFFIC_BYTES_SMALL_MBA = 67.19e6
+# `ncu --set full` capture summarised in profiles/r1c_final.md (48.11 MB + 18.57 MB)
+K1_TRAFFIC_BYTES_SMALL_MBA = 66.68e6
 
 
 def parse_args():
