@@ -472,3 +472,38 @@ def test_streaming_zero_copy_gather_matches_copied_batches(case, expect_auto, mo
             assert st["image_zero_copy"] == want, (mode, st)
         assert (st["h2d_image_bytes"] == 0) == (st["image_zero_copy"] == 1)
         assert np.array_equal(hits_s, hits_r) and np.array_equal(snr_s, snr_r), mode
+
+
+@pytest.mark.parametrize("case", ["neo", "small_mba", "tno", "neo+focused", "small_mba+focused", "tno+focused"])
+def test_precull_is_conservative_at_scale(case):
+    """The pre-cull (cone test on the geometric, possibly unpolished, position) may only drop pairs
+    that cannot hit: dt_stack with and without it (DT_FLAG_NO_PRECULL refines every pair at full
+    precision) must give identical hit counts and SNR for every orbit -- checked on 2e5 orbits x all
+    exposures of the config's survey geometry with small planes (1e8 pairs; eccentric NEOs at all
+    distances included), where any wrongly culled pair would show up."""
+    dt = _dt()
+    base = case.split("+")[0]
+    cfg = ds.scaled(ds.CONFIGS[base], n_orbits=200_000, n_exp=min(ds.CONFIGS[base].n_exp, 500))
+    if case.endswith("+focused"):       # thousands of hits per exposure, many of them near the footprint edge
+        cfg = ds.focused(cfg)
+    sc = ds.build_scene(cfg, oracle.scene_project_fn if case.endswith("+focused") else None, inject=False)
+    el = torch.from_numpy(sc.elements()).cuda()
+    g = torch.Generator(device="cuda")
+    g.manual_seed(3)
+    # one shared random plane stands in for all exposures (pixel values only matter for equality)
+    plane = torch.randn((1, cfg.height, cfg.width), generator=g, device="cuda", dtype=torch.float32)
+    vplane = torch.full_like(plane, 1.25) if cfg.variance_mode == 1 else None
+    out = {}
+    for flags in (0, 4):
+        with dt.Tracker.from_scene(sc, flags=flags, hbm_budget_bytes=cfg.image_bytes() + (1 << 30)) as trk:
+            for j in range(cfg.n_exp):
+                trk.load_image_batch(j, plane, vplane)
+            snr, hits = trk.stack(el, sc.t0)
+            st = trk.stats()
+            out[flags] = (snr.cpu().numpy(), hits.cpu().numpy(), st["hits"], st["refined_pairs"])
+    assert out[0][2] == out[4][2] and out[0][2] > 0, (out[0][2], out[4][2])
+    assert np.array_equal(out[0][1], out[4][1])
+    assert np.array_equal(out[0][0], out[4][0])
+    if not case.endswith("+focused"):
+        assert out[0][3] < 0.05 * out[4][3]      # and it does cull
+    print(case, "hits", out[0][2], "refined pairs with / without the pre-cull", out[0][3], out[4][3])
