@@ -31,16 +31,14 @@ import dtsynth as ds  # noqa: E402
 METRIC = "orbit-exposure pairs/sec (propagate+project+gather+stack)"
 UNIT = "pairs/s"
 # FP64-pipe instructions kernel 1 issues per pair on its two paths,
-# measured with ncu smsp__inst_executed_pipe_fp64.sum on configs[1] (profiles/r1c_final.md): 58.25 per
-# pair with the pre-cull (0.01 % of the pairs refined: order-3 warm Kepler step with the Newton polish
-# deferred, geometric position, cone test) and 130.0 per pair with DT_FLAG_NO_PRECULL (every pair
-# polished and refined; that mode has no cone test, ~6 instructions).  A refined pair therefore costs
-# at least 130 + 6 - 58.25 = 78 more (polish 8 + light-time re-solve, projection, footprint test 70;
-# 11 more when the polish had been deferred and the geometric distance is recomputed).  Other
-# workloads take longer Kepler paths (wide steps on NEO), so the model under-counts their work: their
-# `frac` is a lower bound.
-FP64_SLOTS_COARSE = 58.25    # every pair
-FP64_SLOTS_REFINE = 78.0     # refined pairs only, on top
+# measured with ncu smsp__inst_executed_pipe_fp64.sum on configs[1] (profiles/r1c_final.md): 51.5 per
+# pair with the pre-cull (0.01 % of the pairs refined: cull-quality order-2 warm Kepler step without
+# polish, geometric position, cone test) and 130.0 per pair with DT_FLAG_NO_PRECULL (every pair solved
+# to full precision and refined; that mode has no cone test, ~6 instructions).  A refined pair
+# therefore costs at least 130 + 6 - 51.5 = 84.5 more.  Other workloads take longer Kepler paths (wide
+# steps on NEO), so the model under-counts their work: their `frac` is a lower bound.
+FP64_SLOTS_COARSE = 51.5     # every pair
+FP64_SLOTS_REFINE = 84.5     # refined pairs only, on top
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_propagate<3> launch on configs[1], from the
 # `ncu --set full` capture summarised in profiles/r1c_final.md (48.11 MB + 18.57 MB)
 K1_TRAFFIC_BYTES_SMALL_MBA = 66.68e6

@@ -29,6 +29,7 @@ struct Orbit {
     double n, e, M0;
     double Ax, Ay, Az, Bx, By, Bz;  // equatorial, AU
     double cos2_cull;               // cos^2 of the pre-cull cone half-angle
+    double rho2_close;              // pairs closer than this (AU^2) are always refined
     bool valid;
 };
 
@@ -72,9 +73,14 @@ __device__ __forceinline__ Orbit orbit_setup(const double el_in[6], double gm, d
     // seen by the observer, asin(v_max / c) with v_max the perihelion speed (|r(t) - r(t - tau)| <=
     // v_max tau and tau = rho0 / c exactly, so the bound does not depend on rho0), + slack.
     const double vmax = sqrt(gm / a * (1.0 + e) / (1.0 - e));
-    const double th = atan(tan_fov) * 1.01 + 1.05 * asin(fmin(vmax * inv_c, 1.0)) + 2e-5;
+    const double th = atan(tan_fov) * 1.01 + 1.05 * asin(fmin(vmax * inv_c, 1.0)) + 1.4e-4;
     const double cth = (th < 1.5) ? cos(th) : 0.0;
     o.cos2_cull = (th < 1.5) ? cth * cth : -1.0;  // -1: cone test disabled (always refine)
+    // The cull may run on an UNPOLISHED order-2 Kepler state, off by <= 6e-6 rad in E (k_propagate), i.e.
+    // by <= 6e-6 a AU in position (|dr/dE| <= a) and 6e-6 a / rho in direction: 1e-4 rad of the slack
+    // above are reserved for it, which holds for rho >= 0.06 a; closer pairs (and anything inside
+    // 0.1 AU) are refined unconditionally.
+    o.rho2_close = fmax(0.01, 0.0036 * a * a);
     return o;
 }
 
@@ -230,9 +236,26 @@ __device__ __forceinline__ Kepler kepler_polish(double e, const Kepler &K0)
     return K;
 }
 
+// Two Newton steps on a state that may be off by up to ~1e-5 rad (an unpolished ORDER 2 step): the
+// first with a correctly rounded reciprocal and a third-order rotation by its correction d (d^4/24 <
+// 1e-21), the second first-order (d2 ~ a2 d^2 <= 1e-10).
+__device__ __forceinline__ Kepler kepler_polish2(double e, const Kepler &K0)
+{
+    const double g1 = fma(-e, K0.c, 1.0);
+    const double d = -fma(-e, K0.s, K0.u) * rcp_nr<2>(g1);
+    const double d2h = 0.5 * d * d;                              // 1 - cos d
+    const double sd = fma(-d * d2h, 1.0 / 3.0, d);               // sin d = d - d^3/6
+    Kepler K;
+    K.M = K0.M;
+    K.u = K0.u + d;
+    K.s = K0.s + fma(K0.c, sd, -K0.s * d2h);
+    K.c = K0.c - fma(K0.s, sd, K0.c * d2h);
+    return kepler_polish(e, K);
+}
+
 // POLISH = false returns the state right after the series step and the rotation: a self-consistent
 // point (s = sin(M + u), c = cos(M + u)) whose u is off by the series truncation (<= 6.5e-8 rad for
-// ORDER 3, chained steps included: the next step's series starts from the exact residual of the
+// ORDER 3, <= 4.3e-6 rad for ORDER 2 inside the ORDER 3 domain, chained steps included: the next step's series starts from the exact residual of the
 // state it is given, so the error does not accumulate).  Good enough to CULL with; kepler_polish
 // finishes the job for the pairs that survive.
 template <int ORDER, bool POLISH = true>

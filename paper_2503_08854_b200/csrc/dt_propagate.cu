@@ -129,13 +129,13 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 if (have_state) {
                     const WarmPre w = kepler_warm_pre(o.e, K, M);
                     if (__all_sync(0xffffffffu, kepler_warm_in_domain<3>(w))) {
-                        // with the pre-cull the Newton polish is deferred to the pairs that survive it:
-                        // the unpolished state is off by <= 6.5e-8 rad in E, far inside the cone's slack
-                        // (objects closer than 0.1 AU are always refined, see `near` below)
+                        // with the pre-cull the precision is deferred to the pairs that survive it
                         // (a warp whose last pair survived the cull -- a focused search -- polishes at
                         // once: deferring would cost it the geometric distance twice)
                         if (PRECULL && !prev_refined) {
-                            K = kepler_warm_finish<3, false>(o.e, K, M, w);
+                            // cull quality only: second-order series, no polish (<= 6e-6 rad in E, see
+                            // orbit_setup for the cone slack that pays for it)
+                            K = kepler_warm_finish<2, false>(o.e, K, M, w);
                             unpolished = true;
                         } else {
                             K = kepler_warm_finish<3, true>(o.e, K, M, w);
@@ -196,9 +196,9 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 // conservative cone test on the GEOMETRIC direction (see orbit_setup)
                 const double D0 = fma(dx0, x.tx, fma(dy0, x.ty, dz0 * x.tz));
                 near = !(D0 * D0 < o.cos2_cull * rho2) && (D0 > 0.0 || o.cos2_cull < 0.0);
-                // always refine objects closer than 0.1 AU: there a state error of 6.5e-8 rad in E could
-                // move the direction by more than the cone's 2e-5 rad slack (and rho2 ~ 0 must not cull)
-                near = near || !(rho2 > 0.01);
+                // always refine close objects: there the error of the unpolished state could move the
+                // direction by more than the cone's slack (and rho2 ~ 0 must not cull)
+                near = near || !(rho2 > o.rho2_close);
             }
             bool hit = false;
             int32_t ix = -1, iy = -1;
@@ -210,7 +210,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 double rho2r = rho2;
                 if (unpolished) {
                     // the deferred polish, then the geometric distance again from the polished state
-                    K = kepler_polish(o.e, K);
+                    K = kepler_polish2(o.e, K);
                     const double X0p = K.c - o.e;
                     const double ax0 = fma(o.Ax, X0p, fma(o.Bx, K.s, -x.Rx));
                     const double ay0 = fma(o.Ay, X0p, fma(o.By, K.s, -x.Ry));
