@@ -142,7 +142,14 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                         }
                         solved = true;
                     } else if (__all_sync(0xffffffffu, kepler_warm_in_domain<4>(w))) {
-                        K = kepler_warm_finish<4>(o.e, K, M, w);
+                        if (PRECULL && !prev_refined) {
+                            // cull quality on the order-4 domain: third-order series, no polish
+                            // (<= 3.7e-6 rad in E over chained steps, inside the same 6e-6 budget)
+                            K = kepler_warm_finish<3, false>(o.e, K, M, w);
+                            unpolished = true;
+                        } else {
+                            K = kepler_warm_finish<4>(o.e, K, M, w);
+                        }
                         solved = true;
                     } else {
                         // some lane's step is too long (a long gap, or close to the perihelion of an
