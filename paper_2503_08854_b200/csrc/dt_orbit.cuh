@@ -361,6 +361,8 @@ __device__ __forceinline__ Kepler kepler_warm(double e, const Kepler &K0, double
 // Worst error of (u, sin E, cos E) against 40-digit solutions over 2e4 accepted random steps with
 // e <= 0.9: 6.5e-16 (the narrow step, with its single polish: 1.8e-13).
 // ~75 FP64 instructions against ~45 for the narrow step and several hundred for a cold solve.
+// POLISH2 = false stops after the first polish: <= 5.3e-8 rad in E over chained steps (cull quality).
+template <bool POLISH2 = true>
 __device__ __forceinline__ Kepler kepler_warm_wide_finish(double e, const Kepler &K0, double Mn, const WarmPre &w,
                                                           bool &ok)
 {
@@ -391,6 +393,14 @@ __device__ __forceinline__ Kepler kepler_warm_wide_finish(double e, const Kepler
     const double s2 = s1 + fma(c1, sd, -s1 * d2h);
     const double c2 = c1 - fma(s1, sd, c1 * d2h);
     const double u2 = u1 + d;
+    if (!POLISH2) {
+        Kepler Kc;
+        Kc.M = Mn;
+        Kc.u = u2;
+        Kc.s = s2;
+        Kc.c = c2;
+        return Kc;
+    }
     // polish 2: first order, 1/g2 by one Newton step from 1/g1
     const double g2 = fma(-e, c2, 1.0);
     const double rg2 = rg1 * fma(-g2, rg1, 2.0);
@@ -403,9 +413,10 @@ __device__ __forceinline__ Kepler kepler_warm_wide_finish(double e, const Kepler
     return K;
 }
 
+template <bool POLISH2 = true>
 __device__ __forceinline__ Kepler kepler_warm_wide(double e, const Kepler &K0, double Mn, bool &ok)
 {
-    return kepler_warm_wide_finish(e, K0, Mn, kepler_warm_pre(e, K0, Mn), ok);
+    return kepler_warm_wide_finish<POLISH2>(e, K0, Mn, kepler_warm_pre(e, K0, Mn), ok);
 }
 
 // How far outside kepler_warm_wide's accuracy domain the step of prefix w is: acceptable when the

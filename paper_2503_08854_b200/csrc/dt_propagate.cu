@@ -163,19 +163,24 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                             const int ns = (r <= 0.8f) ? 1 : (int)ceilf(1.3f * r);
                             Kepler Kc = K;
                             bool good = true;
+                            const bool cullq = PRECULL && !prev_refined;   // second polish deferred to survivors
                             if (ns == 1) {
-                                Kc = kepler_warm_wide_finish(o.e, K, M, w, good);
+                                Kc = cullq ? kepler_warm_wide_finish<false>(o.e, K, M, w, good)
+                                           : kepler_warm_wide_finish<true>(o.e, K, M, w, good);
                             } else {
                                 const double M_from = K.M, dMs = (M - M_from) / (double)ns;
                                 for (int sidx = 1; sidx <= ns; ++sidx) {
                                     bool oks;
-                                    Kc = kepler_warm_wide(o.e, Kc, (sidx == ns) ? M : fma(dMs, (double)sidx, M_from), oks);
+                                    const double Ms = (sidx == ns) ? M : fma(dMs, (double)sidx, M_from);
+                                    Kc = cullq ? kepler_warm_wide<false>(o.e, Kc, Ms, oks)
+                                               : kepler_warm_wide<true>(o.e, Kc, Ms, oks);
                                     good = good && oks;
                                 }
                             }
                             if (__all_sync(0xffffffffu, good)) {
                                 K = Kc;
                                 solved = true;
+                                unpolished = cullq;
                                 n_sub += 1;
                             }
                         }
