@@ -31,14 +31,14 @@ import dtsynth as ds  # noqa: E402
 METRIC = "orbit-exposure pairs/sec (propagate+project+gather+stack)"
 UNIT = "pairs/s"
 # FP64-pipe instructions kernel 1 issues per pair on its two paths,
-# measured with ncu smsp__inst_executed_pipe_fp64.sum on configs[1] (profiles/r1c_final.md): 51.5 per
+# measured with ncu smsp__inst_executed_pipe_fp64.sum on configs[1] (profiles/r1c_final.md): 50.0 per
 # pair with the pre-cull (0.01 % of the pairs refined: cull-quality order-2 warm Kepler step without
-# polish, geometric position, cone test) and 130.0 per pair with DT_FLAG_NO_PRECULL (every pair solved
+# polish or refresh, reciprocal from the MUFU seed, geometric position, cone test) and 130.0 per pair with DT_FLAG_NO_PRECULL (every pair solved
 # to full precision and refined; that mode has no cone test, ~6 instructions).  A refined pair
-# therefore costs at least 130 + 6 - 51.5 = 84.5 more.  Other workloads take longer Kepler paths (wide
+# therefore costs at least 130 + 6 - 50.0 = 86.0 more.  Other workloads take longer Kepler paths (wide
 # steps on NEO), so the model under-counts their work: their `frac` is a lower bound.
-FP64_SLOTS_COARSE = 51.5     # every pair
-FP64_SLOTS_REFINE = 84.5     # refined pairs only, on top
+FP64_SLOTS_COARSE = 50.0     # every pair
+FP64_SLOTS_REFINE = 86.0     # refined pairs only, on top
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_propagate<3> launch on configs[1], from the
 # `ncu --set full` capture summarised in profiles/r1c_final.md (48.33 MB + 19.25 MB)
 K1_TRAFFIC_BYTES_SMALL_MBA = 67.58e6

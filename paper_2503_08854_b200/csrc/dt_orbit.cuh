@@ -308,14 +308,17 @@ __device__ __forceinline__ Kepler kepler_warm_tail(double e, const Kepler &K0, d
 struct WarmPre {
     double dM, es, ec, rg, x, a2, ax, axa2;
 };
-__device__ __forceinline__ WarmPre kepler_warm_pre(double e, const Kepler &K0, double Mn)
+// `seed_only` (warp-uniform): 1/g straight from the MUFU seed (1e-6 relative, i.e. <= 3e-7 rad of
+// theta): enough for a cull-quality step.
+__device__ __forceinline__ WarmPre kepler_warm_pre(double e, const Kepler &K0, double Mn, bool seed_only = false)
 {
     WarmPre w;
     w.dM = Mn - K0.M;
     w.es = e * K0.s;
     w.ec = e * K0.c;
     const double f0 = (K0.u - w.es) - w.dM;
-    w.rg = rcp_nr<1>(1.0 - w.ec);            // 1e-12 relative: the polish removes what it costs theta
+    // full steps: one Newton iteration, 1e-12 relative (the polish removes what that costs theta)
+    w.rg = seed_only ? rcp_nr<0>(1.0 - w.ec) : rcp_nr<1>(1.0 - w.ec);
     w.x = -f0 * w.rg;
     w.a2 = 0.5 * w.es * w.rg;
     w.ax = fabs(w.x);
@@ -427,6 +430,19 @@ __device__ __forceinline__ float kepler_warm_need_pre(const WarmPre &w)
     const float lin = (float)fmax(w.ax * (1.0 / 0.3), w.axa2 * (1.0 / 0.08));
     const float cub = sqrtf((float)(fabs(w.ec * w.rg) * w.x * w.x * (1.0 / (6.0 * 0.02))));
     return fmaxf(lin, cub);
+}
+
+// Re-synchronise (sin E, cos E) with E = M + u exactly (libdevice sincos of the reduced angle), u
+// untouched: the survivors of the cull start their polishes from here, so that neither the
+// truncation of the cull-quality rotations nor their rounding can reach a refined pair.
+__device__ __forceinline__ Kepler kepler_resync(const Kepler &K0)
+{
+    const double k = rint(K0.M * kInvTwoPi);
+    double m = fma(-k, kTwoPiHi, K0.M);
+    m = fma(-k, kTwoPiLo, m);
+    Kepler K = K0;
+    sincos(m + K0.u, &K.s, &K.c);
+    return K;
 }
 
 // Refresh: recompute (sin E, cos E) of the carried state exactly (libdevice sincos of the reduced

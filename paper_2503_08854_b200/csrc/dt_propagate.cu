@@ -100,6 +100,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
     K.c = 1.0;
     bool have_state = false;
     bool prev_refined = false;     // warp-uniform: the last exposure's pairs went through the refinement
+    int since_sync = 0;            // warp-uniform: cull-quality steps since (sin E, cos E) were last exact
     unsigned long long n_refined = 0, n_cold = 0, n_hits = 0, n_sub = 0;
 
     for (int g = g_begin; g < g_end; ++g) {
@@ -108,7 +109,12 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
         mbar_wait(&sm.full[slot], parity);
         const int nrec = min(kGroup, p.n_exp - g * kGroup);
 
-        if (WARM && have_state) K = kepler_refresh(o.e, K);
+        // (a warp that is culling needs no refresh: its chain is cull quality and self-correcting, and
+        // the pairs that survive re-synchronise (sin E, cos E) exactly before they are refined)
+        if (WARM && have_state && (!PRECULL || prev_refined)) {
+            K = kepler_refresh(o.e, K);
+            since_sync = 0;
+        }
 
         uint32_t bits = 0;
         int cnt = 0;          // this lane's hits in the group
@@ -127,7 +133,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 bool solved = false;
                 unpolished = false;
                 if (have_state) {
-                    const WarmPre w = kepler_warm_pre(o.e, K, M);
+                    const WarmPre w = kepler_warm_pre(o.e, K, M, PRECULL && !prev_refined);
                     if (__all_sync(0xffffffffu, kepler_warm_in_domain<3>(w))) {
                         // with the pre-cull the precision is deferred to the pairs that survive it
                         // (a warp whose last pair survived the cull -- a focused search -- polishes at
@@ -137,6 +143,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                             // orbit_setup for the cone slack that pays for it)
                             K = kepler_warm_finish<2, false>(o.e, K, M, w);
                             unpolished = true;
+                            since_sync += 1;
                         } else {
                             K = kepler_warm_finish<3, true>(o.e, K, M, w);
                         }
@@ -147,6 +154,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                             // (<= 3.7e-6 rad in E over chained steps, inside the same 6e-6 budget)
                             K = kepler_warm_finish<3, false>(o.e, K, M, w);
                             unpolished = true;
+                            since_sync += 1;
                         } else {
                             K = kepler_warm_finish<4>(o.e, K, M, w);
                         }
@@ -222,6 +230,12 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 double rho2r = rho2;
                 if (unpolished) {
                     // the deferred polish, then the geometric distance again from the polished state
+                    // (sin E, cos E) carry 1.6e-14 of truncation per cull-quality rotation: re-synchronise
+                    // them exactly once more than a few such steps have piled up
+                    if (since_sync > 6) {
+                        K = kepler_resync(K);
+                        since_sync = 0;
+                    }
                     K = kepler_polish2(o.e, K);
                     const double X0p = K.c - o.e;
                     const double ax0 = fma(o.Ax, X0p, fma(o.Bx, K.s, -x.Rx));
