@@ -40,8 +40,8 @@ UNIT = "pairs/s"
 FP64_SLOTS_COARSE = 50.0     # every pair
 FP64_SLOTS_REFINE = 86.0     # refined pairs only, on top
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_propagate<3> launch on configs[1], from the
-# `ncu --set full` capture summarised in profiles/r1c_final.md (48.33 MB + 19.25 MB)
-K1_TRAFFIC_BYTES_SMALL_MBA = 67.58e6
+# `ncu --set full` capture summarised in profiles/r1c_final.md (48.35 MB + 19.71 MB)
+K1_TRAFFIC_BYTES_SMALL_MBA = 68.05e6
 
 
 def parse_args():
