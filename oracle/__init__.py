@@ -41,6 +41,11 @@ class _Survey(C.Structure):
                 ("var_scalar", C.POINTER(C.c_double))]
 
 
+class _StackOpts(C.Structure):
+    _fields_ = [("patch", C.c_int32), ("weights", C.POINTER(C.c_double)), ("clip", C.c_double),
+                ("t0_per_orbit", C.POINTER(C.c_double))]
+
+
 class PairStruct(C.Structure):
     _fields_ = [("M", C.c_double), ("E", C.c_double), ("r", C.c_double * 3), ("tau", C.c_double),
                 ("M1", C.c_double), ("E1", C.c_double), ("r1", C.c_double * 3),
@@ -67,6 +72,10 @@ def lib():
         L.dto_stack.argtypes = [C.POINTER(_Survey), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
                                 dp, C.c_int64, C.c_double, dp, ip, dp, dp, ip]
         L.dto_topk.argtypes = [dp, ip, C.c_int64, C.c_int32, C.c_int32, C.POINTER(C.c_int64), dp, ip]
+        L.dto_stack_ex.argtypes = [C.POINTER(_Survey), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), dp, C.c_int64,
+                                   C.c_double, C.POINTER(_StackOpts), dp, ip, dp, dp, ip]
+        L.dto_threshold.argtypes = [dp, ip, C.c_int64, C.c_double, C.c_int32, C.c_int64, C.POINTER(C.c_int64), dp,
+                                    C.POINTER(C.c_int64)]
         L.dto_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -181,6 +190,44 @@ def stack(survey: Survey, flux, var, elements: np.ndarray, t0: float):
     if rc != 0:
         raise ValueError("dto_stack failed (%d)" % rc)
     return dict(snr=snr, hits=hits, S=S, Wt=Wt, nflag=nflag)
+
+
+def stack_ex(survey: Survey, flux, var, elements: np.ndarray, t0: float = 0.0, patch: int = 1, weights=None,
+             clip: float = float("inf"), t0_per_orbit=None):
+    """Extended stack (dt_oracle.h dto_stack_ex): k x k patch with PSF weights, per-intersection outlier
+    clip, per-orbit epochs.  -> dict(snr, hits, S, Wt, nflag)"""
+    el = np.ascontiguousarray(elements, dtype=np.float64).reshape(-1, 6)
+    n, N = el.shape[0], survey.n_exposures
+    fp, _keep_f = _plane_ptrs(flux, N)
+    vp, _keep_v = _plane_ptrs(var, N)
+    w = np.ascontiguousarray(weights, dtype=np.float64).reshape(-1) if weights is not None else None
+    if w is not None:
+        assert w.size == patch * patch
+    te = np.ascontiguousarray(t0_per_orbit, dtype=np.float64) if t0_per_orbit is not None else None
+    if te is not None:
+        assert te.shape == (n,)
+    opts = _StackOpts(patch, _dp(w) if w is not None else None, clip, _dp(te) if te is not None else None)
+    snr, S, Wt = np.empty(n), np.empty(n), np.empty(n)
+    hits, nflag = np.empty(n, np.int32), np.empty(n, np.int32)
+    ip = C.POINTER(C.c_int32)
+    rc = lib().dto_stack_ex(C.byref(survey._c), fp, vp, _dp(el), n, t0, C.byref(opts), _dp(snr),
+                            hits.ctypes.data_as(ip), _dp(S), _dp(Wt), nflag.ctypes.data_as(ip))
+    if rc != 0:
+        raise ValueError("dto_stack_ex failed (%d)" % rc)
+    return dict(snr=snr, hits=hits, S=S, Wt=Wt, nflag=nflag)
+
+
+def threshold(snr: np.ndarray, hits: np.ndarray, snr_min: float, min_hits: int = 0, max_out: int = 1 << 20):
+    """-> (index, snr, n_found): every orbit with finite snr >= snr_min and hits >= min_hits, index order."""
+    snr = np.ascontiguousarray(snr, dtype=np.float64)
+    hits = np.ascontiguousarray(hits, dtype=np.int32)
+    idx, val, nf = np.empty(max(max_out, 1), np.int64), np.empty(max(max_out, 1)), C.c_int64()
+    rc = lib().dto_threshold(_dp(snr), hits.ctypes.data_as(C.POINTER(C.c_int32)), snr.size, snr_min, min_hits,
+                             max_out, idx.ctypes.data_as(C.POINTER(C.c_int64)), _dp(val), C.byref(nf))
+    if rc != 0:
+        raise ValueError("dto_threshold failed (%d)" % rc)
+    m = min(nf.value, max_out)
+    return idx[:m].copy(), val[:m].copy(), nf.value
 
 
 def topk(snr: np.ndarray, hits: np.ndarray, k: int, min_hits: int = 0):

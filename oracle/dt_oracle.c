@@ -231,6 +231,89 @@ int dto_stack(const dto_survey *s, const float *const *flux, const float *const 
     return 0;
 }
 
+/* SURVEY.md 8(f) NEXT-1 / NEXT-3 (readings A21-A23): patch gather with PSF weights, per-intersection
+ * outlier rejection, per-orbit epochs.  See dt_oracle.h for the definition this follows line by line. */
+int dto_stack_ex(const dto_survey *s, const float *const *flux, const float *const *var,
+                 const double *elements, int64_t n, double t0, const dto_stack_opts *opts,
+                 double *snr, int32_t *hits, double *S_out, double *Wt_out, int32_t *nflag)
+{
+    const int32_t N = s->n_exposures;
+    const int64_t W = s->width, H = s->height;
+    const int32_t k = opts ? opts->patch : 1;
+    if (k < 1 || (k % 2) == 0) return -1;
+    if (s->variance_mode == 1 && var == NULL) return -1;
+    const int32_t h = k / 2;
+    const double clip = opts ? opts->clip : INFINITY;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t o = 0; o < n; ++o) {
+        const double *el = elements + 6 * o;
+        const double t0o = (opts && opts->t0_per_orbit) ? opts->t0_per_orbit[o] : t0;
+        if (!valid_orbit(el) || !isfinite(t0o)) {
+            if (snr) snr[o] = NAN;
+            if (hits) hits[o] = -1;
+            if (S_out) S_out[o] = NAN;
+            if (Wt_out) Wt_out[o] = NAN;
+            if (nflag) nflag[o] = 0;
+            continue;
+        }
+        double S = 0.0, Wt = 0.0;
+        int32_t nh = 0, nf = 0;
+        for (int32_t j = 0; j < N; ++j) {
+            dto_pair p;
+            dto_pair_chain(s, el, t0o, j, &p);
+            if (p.flag && p.D > 0.0 && p.x + 0.5 >= -1.0 && p.x + 0.5 < (double)s->width + 1.0 &&
+                p.y + 0.5 >= -1.0 && p.y + 0.5 < (double)s->height + 1.0)
+                nf += 1;
+            if (!p.hit) continue;
+            double si = 0.0, wti = 0.0;
+            int32_t used = 0;
+            for (int32_t dy = -h; dy <= h; ++dy) {
+                for (int32_t dx = -h; dx <= h; ++dx) {
+                    const int64_t yy = (int64_t)p.iy + dy, xx = (int64_t)p.ix + dx;
+                    if (yy < 0 || yy >= H || xx < 0 || xx >= W) continue;
+                    const int64_t off = yy * W + xx;
+                    const double f = (double)flux[j][off];
+                    const double v = (s->variance_mode == 1) ? (double)var[j][off] : s->var_scalar[j];
+                    if (!(isfinite(f) && isfinite(v) && v > 0.0)) continue;
+                    const double w = (opts && opts->weights) ? opts->weights[(dy + h) * k + (dx + h)] : 1.0;
+                    si += (w * f) / v;
+                    wti += (w * w) / v;
+                    used += 1;
+                }
+            }
+            if (used == 0) continue;
+            if (si > clip * sqrt(wti)) continue;
+            S += si;
+            Wt += wti;
+            nh += 1;
+        }
+        if (snr) snr[o] = (nh > 0) ? S / sqrt(Wt) : 0.0;
+        if (hits) hits[o] = nh;
+        if (S_out) S_out[o] = S;
+        if (Wt_out) Wt_out[o] = Wt;
+        if (nflag) nflag[o] = nf;
+    }
+    return 0;
+}
+
+/* Threshold mode (reading A24): plain scan in ascending orbit index. */
+int dto_threshold(const double *snr, const int32_t *hits, int64_t n, double snr_min, int32_t min_hits,
+                  int64_t max_out, int64_t *index_out, double *snr_out, int64_t *n_found)
+{
+    if (max_out < 0 || !n_found) return -1;
+    int64_t m = 0;
+    for (int64_t o = 0; o < n; ++o) {
+        if (!(isfinite(snr[o]) && snr[o] >= snr_min && hits[o] >= min_hits)) continue;
+        if (m < max_out) {
+            if (index_out) index_out[m] = o;
+            if (snr_out) snr_out[m] = snr[o];
+        }
+        ++m;
+    }
+    *n_found = m;
+    return 0;
+}
+
 /* Step 11 (8(c).11): full sort, SNR descending, ties by orbit index ascending. */
 typedef struct { double snr; int64_t idx; } dto_cand;
 

@@ -18,7 +18,8 @@
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): P1 Kepler residual, P2 Kepler values,
  * P3 circular closed form, P4 invariants, P5 light-time closed form, P6 frame + sky closed form,
  * P7 gnomonic identities, P8 worked example WE-1, P9 stack identities / brute force / injected
- * source recovery, P10 top-k vs full sort.  Parity unpinned: anything about real ZTF pixels,
+ * source recovery, P10 top-k vs full sort, A11 guard-band flag and nflag, P11 extended stack (patch,
+ * outlier clip, per-orbit epochs) and threshold mode (tests/test_oracle_next.py).  Parity unpinned: anything about real ZTF pixels,
  * Chiron's recovered SNR, the Fig. 3 histogram (data and the paper's Python pipeline are missing).
  *
  * Units: AU, days, radians.
@@ -86,6 +87,37 @@ int dto_project(const dto_survey *s, const double *elements, int64_t n, double t
 int dto_stack(const dto_survey *s, const float *const *flux, const float *const *var,
               const double *elements, int64_t n, double t0,
               double *snr, int32_t *hits, double *S, double *Wt, int32_t *nflag);
+
+/* ---- SURVEY.md 8(f) NEXT rows (readings A21-A24 of DESIGN.md; the paper gives prose only) -------------
+ * Options of the extended stack.  For every intersection i (a pair that passes the footprint test of
+ * step 8, nearest pixel (ix, iy)) the k x k patch of pixels centred on (ix, iy) is read ("a
+ * patch of pixels is pulled from the associated image"), row by row (dy ascending, then dx ascending):
+ *     for each patch pixel p inside the image with finite f_p, v_p and v_p > 0:
+ *         s_i += (w_p * f_p) / v_p;   wt_i += (w_p * w_p) / v_p;          (s_i, wt_i start at 0)
+ * (matched filter with caller-supplied PSF weights w[k*k], row-major; v_p is the exposure's scalar in
+ * variance mode 0).  The intersection is skipped (not counted) when no patch pixel contributed, or when
+ * its own SNR is anomalously high ("Intersections with anomalously high SNR value compared
+ * to the expectation can be removed"):  s_i > clip * sqrt(wt_i)  (clip = +inf: never).  Otherwise, in
+ * ascending exposure order, S += s_i; Wt += wt_i; hits += 1.  SNR = S / sqrt(Wt), 0 without hits.
+ * patch = 1, weights = {1}, clip = +inf, t0_per_orbit = NULL is dto_stack bit for bit.
+ * t0_per_orbit ("six orbital elements and an orbital epoch"): epoch of orbit o's M0, or NULL
+ * for the scalar t0 argument. */
+typedef struct {
+    int32_t patch;                /* k >= 1, odd */
+    const double *weights;        /* [k*k] row-major (dy, dx); NULL => all 1 */
+    double clip;                  /* +inf => no rejection */
+    const double *t0_per_orbit;   /* [n] or NULL */
+} dto_stack_opts;
+
+int dto_stack_ex(const dto_survey *s, const float *const *flux, const float *const *var,
+                 const double *elements, int64_t n, double t0, const dto_stack_opts *opts,
+                 double *snr, int32_t *hits, double *S, double *Wt, int32_t *nflag);
+
+/* Threshold mode of `FindSignificantResults` (Alg. 1; "detections above an SNR of 5",
+ * PAPER.md:336): every orbit with finite snr >= snr_min and hits >= min_hits, in ascending orbit index.
+ * *n_found = how many there are; the first min(*n_found, max_out) are written. */
+int dto_threshold(const double *snr, const int32_t *hits, int64_t n, double snr_min, int32_t min_hits,
+                  int64_t max_out, int64_t *index_out, double *snr_out, int64_t *n_found);
 
 /* step 11: k largest SNR among orbits with hits >= min_hits and finite SNR; ties by index. */
 int dto_topk(const double *snr, const int32_t *hits, int64_t n, int32_t k, int32_t min_hits,

@@ -243,6 +243,78 @@ def test_p7_gnomonic_identities():
         assert (ph.ix, ph.iy) == (want, 128)
 
 
+# ---- A11: the guard band (the tolerance of every GPU pixel comparison) ------------------------------------
+def _place(ra0, dec0, W, H, xh, yh):
+    """Elements of an object whose x + 1/2 = xh, y + 1/2 = yh on the tangent plane about (ra0, dec0):
+    textbook inverse TAN, observer at the Sun, no light-time (independent of the oracle's forward chain)."""
+    xi, eta = (xh - 0.5 - (W - 1) / 2) * S, (yh - 0.5 - (H - 1) / 2) * S
+    den = math.cos(dec0) - eta * math.sin(dec0)
+    ra = ra0 + math.atan2(xi, den)
+    dec = math.atan2(math.sin(dec0) + eta * math.cos(dec0), math.hypot(xi, den))
+    return _sun_centred(ra, dec)
+
+
+def test_a11_guard_band_flag_is_1e6_px():
+    """flag == 1 iff frac(x + 1/2) or frac(y + 1/2) lies within 1e-6 of 0 or 1 (reading A11, north_star:
+    "within 1e-6 px of a rounding boundary").  Pairs are placed 5e-7 px (must flag) and 2e-6 px (must
+    not) from a boundary, on either side, in x and in y, inside the image and at its four edges; the
+    placement is checked to 1e-7 px on the oracle's own coordinate first, so a band of 1e-5 (or 1e-7)
+    instead of 1e-6 fails here."""
+    W, H = 256, 192
+    ra0, dec0 = 1.0, 0.5
+    sv = survey(0.0, ra0, dec0, W, H, obs=np.zeros((1, 3)), c=float("inf"))
+    n_checked = 0
+    for axis in (0, 1):
+        size = W if axis == 0 else H
+        for k in (0, 1, 57, size - 1, size):          # both footprint edges are rounding boundaries too
+            for d, want in [(5e-7, 1), (-5e-7, 1), (2e-6, 0), (-2e-6, 0), (0.3, 0)]:
+                other = 100.37                          # the other coordinate sits well inside a pixel
+                xh, yh = (k + d, other) if axis == 0 else (other, k + d)
+                p = oracle.pair(sv, _place(ra0, dec0, W, H, xh, yh), 0.0, 0)
+                got = (p.x + 0.5, p.y + 0.5)
+                assert abs(got[0] - xh) < 1e-7 and abs(got[1] - yh) < 1e-7, "placement"
+                assert p.flag == want, (axis, k, d, p.flag)
+                # the flag never changes the hit decision: half-open footprint, floor(x + 1/2)
+                inside = 0.0 <= xh < W and 0.0 <= yh < H
+                assert p.hit == int(inside)
+                if inside:
+                    assert (p.ix, p.iy) == (math.floor(xh), math.floor(yh))
+                n_checked += 1
+    assert n_checked == 50
+    # both coordinates at once, and the project() array output carries the same flag
+    els = [_place(ra0, dec0, W, H, 10 + 5e-7, 20 - 5e-7), _place(ra0, dec0, W, H, 10.5, 20.5)]
+    out = oracle.project(sv, np.array(els), 0.0)
+    assert out["flag"].tolist() == [[1], [0]]
+    # behind the observer nothing is flagged
+    pb = oracle.pair(sv, _sun_centred(ra0 + math.pi, -dec0), 0.0, 0)
+    assert pb.D < 0 and pb.flag == 0
+
+
+def test_a11_stack_counts_flagged_pairs_per_orbit():
+    """dto_stack's nflag (what the GPU parity tests use to excuse an orbit): the number of the orbit's
+    pairs that are flagged in or next to the footprint.  Scene: three exposures one day apart with the
+    same tangent point on a 16384^2 image, observer at the Sun, no light-time; orbit A is placed 5e-7 px
+    from a rounding boundary in exposure 0 and moves ~3400 px per day (unflagged, still inside, in
+    exposures 1 and 2); orbit B sits 2e-6 px from the same boundary; orbit C is flagged but two pixels
+    outside the footprint (not counted)."""
+    W = H = 16384
+    ra0, dec0 = 2.0, -0.3
+    t = np.array([0.0, 1.0, 2.0])
+    sv = oracle.Survey(t, np.zeros((3, 3)), np.full(3, ra0), np.full(3, dec0), W, H, S, GM, float("inf"), EPS,
+                       0, np.ones(3))
+    els = np.array([_place(ra0, dec0, W, H, 8000 + 5e-7, 8100.4),
+                    _place(ra0, dec0, W, H, 8000 + 2e-6, 8100.4),
+                    _place(ra0, dec0, W, H, -2.0 + 5e-7, 8100.4)])
+    planes = [np.ones((H, W), np.float32)] * 3
+    ref = oracle.stack(sv, planes, None, els, 0.0)
+    flags = oracle.project(sv, els, 0.0)["flag"]
+    assert flags[0, 0] == 1 and flags[1, 0] == 0 and flags[2, 0] == 1
+    assert ref["hits"][0] == 3 and ref["hits"][1] == 3, ref["hits"]
+    assert ref["nflag"].tolist() == [int(flags[0].sum()), int(flags[1].sum()), 0]
+    assert ref["nflag"][0] == 1 and ref["nflag"][1] == 0
+    assert abs(ref["snr"][0] - math.sqrt(3.0)) < 1e-15
+
+
 # ---- P8: worked example --------------------------------------------------------------------------------
 def test_p8_worked_example_we1():
     vals, consts = read_golden("we1.txt")
