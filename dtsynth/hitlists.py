@@ -61,7 +61,7 @@ def build(n_orbits: int, n_groups: int, width: int, height: int, cluster: int, d
             off = py * width + px
             lane_rank = torch.cumsum(on2, 1) - on2
             pos = (seg[g, :, b].unsqueeze(1) + lane_rank).reshape(-1)[on]
-            offsets[pos] = off.to(torch.int32)
+            offsets[pos] = (off + (b << 27)).to(torch.int32)      # entry = (exposure in group) << 27 | pixel offset
             sec_ids.append(torch.unique((j * plane + off) >> 3))          # 8 fp32 per 32-B sector
         if sec_ids:
             sectors += int(sum(s.numel() for s in sec_ids))               # exposures are disjoint

@@ -60,8 +60,12 @@ enum {
     DT_FLAG_FORCE_STREAM = 1,   /* never keep images resident: always stream batches from host     */
     DT_FLAG_KEPLER_COLD = 2,    /* solve every pair from a cold start with libdevice sincos        */
                                 /* (reference mode of kernel 1; default is the warm-started solve) */
-    DT_FLAG_NO_PRECULL = 4      /* do the light-time refinement + projection for every pair, even  */
+    DT_FLAG_NO_PRECULL = 4,     /* do the light-time refinement + projection for every pair, even  */
                                 /* when a conservative cone test already proves a miss             */
+    DT_FLAG_PROJECT_PRECULL = 8 /* dt_project runs kernel 1 exactly as dt_stack does, pre-cull and */
+                                /* cull-quality Kepler chain included: a pair the cone test rejects */
+                                /* is reported as culled (NaN, (-1,-1)).  For parity tests of the   */
+                                /* path the timed kernel takes; default dt_project refines all.    */
 };
 
 /*
@@ -72,7 +76,7 @@ enum {
 typedef struct {
     uint32_t struct_size;      /* sizeof(dt_survey): ABI versioning, must match                   */
     int32_t n_exposures;       /* N >= 1                                                          */
-    int32_t width, height;     /* pixels; 1 <= W, H and W*H < 2^31                                */
+    int32_t width, height;     /* pixels; 1 <= W, H and W*H <= 2^27                               */
     const double *t;           /* [N] exposure mid-times, days                                    */
     const double *obs_ecl;     /* [N][3] heliocentric ECLIPTIC observer position at t[j], AU      */
     const double *ra0;         /* [N] tangent point right ascension, rad                          */
@@ -157,6 +161,48 @@ int dt_stack(dt_context *ctx, const double *elements, int64_t n, double t0, int3
              double *snr_out, int32_t *hits_out);
 
 /*
+ * dt_stack_epochs: dt_stack with ONE EPOCH PER ORBIT ("each of these curves is parametrized by six orbital
+ * elements and an orbital epoch"): t0 [n] fp64, in the same memory
+ * kind as `elements`; M = M0[o] + n[o] (t_j - t0[o]).  A non-finite epoch makes the orbit invalid
+ * (hits = -1, snr = NaN).  Everything else as dt_stack.
+ */
+int dt_stack_epochs(dt_context *ctx, const double *elements, const double *t0, int64_t n, int32_t mem_kind,
+                    double *snr_out, int32_t *hits_out);
+
+/*
+ * dt_set_patch: gather a k x k PATCH of pixels per intersection instead of the nearest pixel ("for each
+ * valid intersection returned, a patch of pixels is pulled from the associated image", PAPER.md:143;
+ * SURVEY.md 8(f) NEXT-1).  k odd, 1 .. 15; weights: HOST [k*k] fp64, row-major (dy, then dx), e.g. the PSF
+ * sampled on the pixel grid, copied by the call; NULL = all 1.  For every intersection (nearest pixel
+ * (ix, iy) inside the footprint), over the patch pixels p inside the image with finite f_p, v_p > 0, row by
+ * row:  s_i += (w_p f_p) / v_p,  wt_i += (w_p w_p) / v_p;  an intersection without any valid pixel is
+ * skipped, otherwise (subject to dt_set_outlier_clip) S += s_i, Wt += wt_i, hits += 1 in ascending exposure
+ * order; SNR = S / sqrt(Wt).  k = 1 with NULL weights (the default) is the single-pixel stack, bit for bit.
+ * Applies to the following dt_stack / dt_stack_epochs / dt_gather_hits calls.
+ */
+int dt_set_patch(dt_context *ctx, int32_t k, const double *weights);
+
+/*
+ * dt_set_outlier_clip: per-intersection outlier rejection ("Intersections with anomalously high SNR value
+ * compared to the expectation can be removed"): an intersection whose
+ * own SNR s_i / sqrt(wt_i) exceeds `clip` (tested as s_i > clip * sqrt(wt_i); single pixel: f/v >
+ * clip * sqrt(1/v)) is dropped before the sums and not counted.  One-sided; +inf (default) switches it
+ * off; NaN is DT_ERR_INVALID_ARG.
+ */
+int dt_set_outlier_clip(dt_context *ctx, double clip);
+
+/*
+ * dt_threshold: threshold mode of `FindSignificantResults` (Algorithm 1; "detections above an
+ * SNR of 5"): every orbit of the most recent dt_stack with finite SNR >= snr_min and
+ * hits >= min_hits, in ascending orbit index.  *n_found = how many there are; the first
+ * min(*n_found, max_out) are written to the HOST arrays index_out [max_out] int64 and snr_out [max_out]
+ * fp64 (snr_out may be NULL).  Errors: DT_ERR_STATE without a dt_stack result; DT_ERR_INVALID_ARG for NaN
+ * snr_min or max_out < 0.
+ */
+int dt_threshold(dt_context *ctx, double snr_min, int32_t min_hits, int64_t max_out, int64_t *index_out,
+                 double *snr_out, int64_t *n_found);
+
+/*
  * dt_topk: the k largest SNR of the most recent dt_stack, SNR descending, ties by orbit index
  * ascending, over orbits with hits >= min_hits and finite SNR (Algorithm 1 `FindSignificantResults`,
  * PAPER.md:173).  index_out [k] int64, snr_out [k] fp64 are HOST pointers; *n_found = min(k, count).
@@ -168,8 +214,10 @@ int dt_topk(dt_context *ctx, int32_t k, int32_t min_hits, int64_t *index_out, do
 /*
  * dt_project: parity/debug entry (not on the timed path): steps 1-6 for every pair, written densely.
  *   radec_out [n][N][2] (alpha in [0, 2pi), delta), xy_out [n][N][2] (x, y), pix_out [n][N][2]
- *   ((-1,-1) when culled).  HOST pointers; any may be NULL.  Uses the same device functions as
- *   dt_stack's kernel 1 (mode selected by the context flags).
+ *   ((-1,-1) when culled).  HOST pointers; any may be NULL.  Uses the same kernel template as
+ *   dt_stack's kernel 1 (Kepler mode selected by the context flags); every pair is refined unless
+ *   DT_FLAG_PROJECT_PRECULL is set, in which case the conservative pre-cull of dt_stack is kept and
+ *   the pairs it rejects come back as NaN / (-1,-1).
  */
 int dt_project(dt_context *ctx, const double *elements, int64_t n, double t0, double *radec_out,
                double *xy_out, int32_t *pix_out);
@@ -179,9 +227,9 @@ int dt_project(dt_context *ctx, const double *elements, int64_t n, double t0, do
  * The hit list uses the library's internal format for ONE exposure range
  * [first_exposure, first_exposure + 32*n_groups): for group g and orbit o, bit b of
  * mask[g*n_pad + o] says orbit o hits exposure first_exposure + 32 g + b; the pixel offsets
- * (iy*W + ix) of warp-tile w = o/32 in group g start at offsets[base[g*(n_pad/32) + w]] and are
- * ordered exposure-ascending, then orbit-ascending inside the tile (so the hits of one exposure
- * are contiguous).  n_pad = n rounded up to 32; n <= 2^20, n_groups <= 16, fewer than 2^32 hits.
+ * of warp-tile w = o/32 in group g start at offsets[base[g*(n_pad/32) + w]] and are ordered
+ * exposure-ascending, then orbit-ascending inside the tile (so the hits of one exposure are
+ * contiguous); an entry is (b << 27) | (iy*W + ix): it carries its exposure b within the group.  n_pad = n rounded up to 32; n <= 2^20, n_groups <= 16, fewer than 2^32 hits.
  * n_hits = number of entries of `offsets` (the kernel picks its dense lock-step or its sparse
  * schedule from the hit density).  All pointers are DEVICE pointers.
  * Accumulates into S[n], Wt[n] (fp64) and cnt[n] (int32), which the caller zero-initialises.
@@ -190,6 +238,35 @@ int dt_project(dt_context *ctx, const double *elements, int64_t n, double t0, do
 int dt_gather_hits(dt_context *ctx, int64_t n, int32_t first_exposure, int32_t n_groups,
                    const uint32_t *mask, const uint64_t *base, const uint32_t *offsets,
                    int64_t n_hits, double *S, double *Wt, int32_t *cnt);
+
+/*
+ * dt_filter_intersections: kernel 1 (+2) alone -- Algorithm 1 `SearchImages` + `FilterGPUIntersections`
+ * -- for ONE work unit: orbits [0, n), n <= 2^20, against exposures
+ * [first_exposure, first_exposure + n_exposures), n_exposures <= 512.  Needs no images.  Exposes the
+ * compacted hit list in the format dt_gather_hits takes: *mask, *base, *offsets are DEVICE pointers
+ * owned by the context, valid until the next dt_stack / dt_filter_intersections / dt_destroy on it;
+ * *n_hits entries of *offsets, *n_pad = n rounded up to 32, *n_groups = ceil(n_exposures / 32).
+ * Used by bench.py to time kernel 3 alone on the hit lists the search really produces and to count
+ * their unique 32-B sectors (the bytes_min of the gather roofline).  Synchronises the context stream.
+ */
+int dt_filter_intersections(dt_context *ctx, const double *elements, int64_t n, double t0, int32_t mem_kind,
+                            int32_t first_exposure, int32_t n_exposures, const uint32_t **mask,
+                            const uint64_t **base, const uint32_t **offsets, int64_t *n_hits, int64_t *n_pad,
+                            int32_t *n_groups);
+
+/*
+ * dt_set_option: tuning knobs of a context (none changes any result; defaults are the measured best).
+ *   "gather_schedule"     -1 chosen on the device from the hit density (default), 0 orbit-major walk,
+ *                         1 dense lock-step (one exposure at a time)
+ *   "gather_window"       dense schedule: exposures the fastest CTA may be ahead (0 = from the L2 size)
+ *   "gather_prefetch"     dense schedule: planes ahead of the L2 prefetch sweep (0 = off)
+ *   "gather_l1"           dense schedule: 1 pixel loads allocate in L1, 0 they do not
+ *   "stream_zero_copy"    streaming mode: -1 probe the hit density (default), 0 always copy batches, 1 always
+ *                         gather from the pinned planes
+ *   "zero_copy_elements"  1 kernel 1 reads DT_MEM_PINNED elements in place (default), 0 copies them first
+ * Errors: DT_ERR_INVALID_ARG for an unknown name or a value out of range.
+ */
+int dt_set_option(dt_context *ctx, const char *name, int64_t value);
 
 int dt_get_stats(const dt_context *ctx, dt_stats *out);
 const char *dt_last_error(const dt_context *ctx);

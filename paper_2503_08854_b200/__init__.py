@@ -23,12 +23,13 @@ from . import _build
 
 DT_OK, DT_ERR_INVALID_ARG, DT_ERR_OOM, DT_ERR_CUDA, DT_ERR_NOT_LOADED, DT_ERR_STATE = 0, -1, -2, -3, -4, -5
 DT_MEM_HOST, DT_MEM_PINNED, DT_MEM_DEVICE = 0, 1, 2
-DT_FLAG_FORCE_STREAM, DT_FLAG_KEPLER_COLD, DT_FLAG_NO_PRECULL = 1, 2, 4
+DT_FLAG_FORCE_STREAM, DT_FLAG_KEPLER_COLD, DT_FLAG_NO_PRECULL, DT_FLAG_PROJECT_PRECULL = 1, 2, 4, 8
 _ERR_NAMES = {-1: "DT_ERR_INVALID_ARG", -2: "DT_ERR_OOM", -3: "DT_ERR_CUDA", -4: "DT_ERR_NOT_LOADED",
               -5: "DT_ERR_STATE"}
 
-EXPORTS = ["dt_create", "dt_destroy", "dt_load_image_batch", "dt_stack", "dt_topk", "dt_project",
-           "dt_gather_hits", "dt_get_stats", "dt_last_error", "dt_version", "dt_fp64_peak"]
+EXPORTS = ["dt_create", "dt_destroy", "dt_load_image_batch", "dt_stack", "dt_stack_epochs", "dt_set_patch",
+           "dt_set_outlier_clip", "dt_threshold", "dt_topk", "dt_project",
+           "dt_gather_hits", "dt_filter_intersections", "dt_set_option", "dt_get_stats", "dt_last_error", "dt_version", "dt_fp64_peak"]
 
 
 class DtError(RuntimeError):
@@ -73,9 +74,17 @@ def lib():
         L.dt_destroy.argtypes = [vp]
         L.dt_load_image_batch.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, C.c_int32]
         L.dt_stack.argtypes = [vp, vp, C.c_int64, C.c_double, C.c_int32, vp, vp]
+        L.dt_stack_epochs.argtypes = [vp, vp, vp, C.c_int64, C.c_int32, vp, vp]
+        L.dt_set_patch.argtypes = [vp, C.c_int32, dp]
+        L.dt_set_outlier_clip.argtypes = [vp, C.c_double]
+        L.dt_threshold.argtypes = [vp, C.c_double, C.c_int32, C.c_int64, C.POINTER(C.c_int64), dp, C.POINTER(C.c_int64)]
         L.dt_topk.argtypes = [vp, C.c_int32, C.c_int32, C.POINTER(C.c_int64), dp, ip]
         L.dt_project.argtypes = [vp, dp, C.c_int64, C.c_double, dp, dp, ip]
         L.dt_gather_hits.argtypes = [vp, C.c_int64, C.c_int32, C.c_int32, vp, vp, vp, C.c_int64, vp, vp, vp]
+        L.dt_filter_intersections.argtypes = [vp, vp, C.c_int64, C.c_double, C.c_int32, C.c_int32, C.c_int32,
+                                              C.POINTER(vp), C.POINTER(vp), C.POINTER(vp),
+                                              C.POINTER(C.c_int64), C.POINTER(C.c_int64), ip]
+        L.dt_set_option.argtypes = [vp, C.c_char_p, C.c_int64]
         L.dt_get_stats.argtypes = [vp, C.POINTER(dt_stats)]
         L.dt_last_error.argtypes = [vp]
         L.dt_last_error.restype = C.c_char_p
@@ -157,7 +166,7 @@ def dt_load_image_batch(ctx, first_exposure: int, flux, var=None) -> None:
     _check(lib().dt_load_image_batch(ctx, first_exposure, count, pf, pv, kind), ctx)
 
 
-def dt_stack(ctx, elements, t0: float, out=None):
+def dt_stack(ctx, elements, t0, out=None):
     """elements [n, 6] float64 (numpy or torch, host or CUDA) -> (snr [n] f64, hits [n] i32) in the
     same kind of container.  `out` = (snr, hits) supplies the output buffers (same memory kind as the
     elements: e.g. pinned torch tensors reused from call to call, so that the device->host copy does not
@@ -189,8 +198,39 @@ def dt_stack(ctx, elements, t0: float, out=None):
             raise ValueError("elements must be float64")
         snr, hits = np.empty(n, np.float64), np.empty(n, np.int32)
         ps, ph = snr.ctypes.data, hits.ctypes.data
-    _check(lib().dt_stack(ctx, pe, n, float(t0), kind, ps, ph), ctx)
+    if not (hasattr(t0, "shape") and len(t0.shape) > 0):
+        _check(lib().dt_stack(ctx, pe, n, float(t0), kind, ps, ph), ctx)
+    else:                                # one epoch per orbit: dt_stack_epochs
+        pt, kind_t = _ptr_kind(t0)
+        host = (DT_MEM_HOST, DT_MEM_PINNED)
+        if int(t0.shape[0]) != n or str(t0.dtype).split(".")[-1] != "float64":
+            raise ValueError("per-orbit epochs: [n] float64")
+        if not (kind_t == kind or (kind in host and kind_t in host)):
+            raise ValueError("epochs must live in the same kind of memory as the elements")
+        if kind == DT_MEM_PINNED and kind_t != DT_MEM_PINNED:
+            kind = DT_MEM_HOST
+        _check(lib().dt_stack_epochs(ctx, pe, pt, n, kind, ps, ph), ctx)
     return snr, hits
+
+
+def dt_set_patch(ctx, k: int, weights=None) -> None:
+    w = np.ascontiguousarray(weights, dtype=np.float64).reshape(-1) if weights is not None else None
+    if w is not None and w.size != k * k:
+        raise ValueError("weights must have k*k entries")
+    _check(lib().dt_set_patch(ctx, k, _dp(w) if w is not None else None), ctx)
+
+
+def dt_set_outlier_clip(ctx, clip: float) -> None:
+    _check(lib().dt_set_outlier_clip(ctx, float(clip)), ctx)
+
+
+def dt_threshold(ctx, snr_min: float, min_hits: int = 0, max_out: int = 1 << 20):
+    """-> (index [m] int64, snr [m] f64, n_found): orbits with SNR >= snr_min, ascending index."""
+    idx, val, nf = np.empty(max(max_out, 1), np.int64), np.empty(max(max_out, 1), np.float64), C.c_int64(0)
+    _check(lib().dt_threshold(ctx, float(snr_min), min_hits, max_out, idx.ctypes.data_as(C.POINTER(C.c_int64)),
+                              _dp(val), C.byref(nf)), ctx)
+    m = min(nf.value, max_out)
+    return idx[:m].copy(), val[:m].copy(), nf.value
 
 
 def dt_topk(ctx, k: int, min_hits: int = 0):
@@ -219,6 +259,23 @@ def dt_gather_hits(ctx, n: int, first_exposure: int, n_groups: int, mask, base, 
             raise ValueError("dt_gather_hits takes contiguous CUDA tensors")
     _check(lib().dt_gather_hits(ctx, n, first_exposure, n_groups, mask.data_ptr(), base.data_ptr(),
                                 offsets.data_ptr(), n_hits, S.data_ptr(), Wt.data_ptr(), cnt.data_ptr()), ctx)
+
+
+def dt_filter_intersections(ctx, elements, t0: float, first_exposure: int, n_exposures: int) -> dict:
+    """Kernel 1 (+2) for one work unit -> dict(mask, base, offsets: device addresses owned by the context,
+    n_hits, n_pad, n_groups); see dtrack.h."""
+    pe, kind = _ptr_kind(elements)
+    m, b, o = C.c_void_p(), C.c_void_p(), C.c_void_p()
+    nh, npad, ng = C.c_int64(), C.c_int64(), C.c_int32()
+    _check(lib().dt_filter_intersections(ctx, pe, int(elements.shape[0]), float(t0), kind, first_exposure,
+                                         n_exposures, C.byref(m), C.byref(b), C.byref(o), C.byref(nh),
+                                         C.byref(npad), C.byref(ng)), ctx)
+    return dict(mask=m.value, base=b.value, offsets=o.value, n_hits=nh.value, n_pad=npad.value,
+                n_groups=ng.value)
+
+
+def dt_set_option(ctx, name: str, value: int) -> None:
+    _check(lib().dt_set_option(ctx, name.encode(), int(value)), ctx)
 
 
 def dt_get_stats(ctx) -> dict:
@@ -256,6 +313,15 @@ class Tracker:
     def stack(self, elements, t0=0.0, out=None):
         return dt_stack(self.ctx, elements, t0, out)
 
+    def set_patch(self, k, weights=None):
+        dt_set_patch(self.ctx, k, weights)
+
+    def set_outlier_clip(self, clip):
+        dt_set_outlier_clip(self.ctx, clip)
+
+    def threshold(self, snr_min, min_hits=0, max_out=1 << 20):
+        return dt_threshold(self.ctx, snr_min, min_hits, max_out)
+
     def topk(self, k, min_hits=0):
         return dt_topk(self.ctx, k, min_hits)
 
@@ -264,6 +330,13 @@ class Tracker:
 
     def gather_hits(self, n, first_exposure, n_groups, mask, base, offsets, n_hits, S, Wt, cnt):
         dt_gather_hits(self.ctx, n, first_exposure, n_groups, mask, base, offsets, n_hits, S, Wt, cnt)
+
+    def filter_intersections(self, elements, t0=0.0, first_exposure=0, n_exposures=None):
+        ne = min(self.n_exposures - first_exposure, 512) if n_exposures is None else n_exposures
+        return dt_filter_intersections(self.ctx, elements, t0, first_exposure, ne)
+
+    def set_option(self, name, value):
+        dt_set_option(self.ctx, name, value)
 
     def stats(self):
         return dt_get_stats(self.ctx)

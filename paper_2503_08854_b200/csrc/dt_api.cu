@@ -59,6 +59,12 @@ struct dt_context {
     // orbit-side buffers
     double *d_el = nullptr;
     int64_t el_cap = 0;
+    double *d_t0 = nullptr;                             // per-orbit epochs of dt_stack_epochs
+    int64_t t0_cap = 0;
+    // extended stack (dt_set_patch, dt_set_outlier_clip)
+    int32_t patch = 1;
+    double *d_patch_w = nullptr;                        // [patch * patch] or NULL (all 1)
+    double clip = INFINITY;
     double *d_S = nullptr, *d_Wt = nullptr, *d_snr = nullptr;
     int32_t *d_cnt = nullptr, *d_hits = nullptr;
     int64_t acc_cap = 0, n_last = -1;
@@ -69,12 +75,13 @@ struct dt_context {
     unsigned long long *d_counters = nullptr;           // [8]
     int *d_progress = nullptr;                          // kernel 3 lock-step counters, one per exposure of a unit
     int32_t gather_window = 1;                          // exposures the slowest and fastest CTA may be apart
-    int32_t gather_lockstep = -1;                       // -1: decided on the device from the hit density
+    int32_t gather_lockstep = -1;                       // schedule: -1 decided on the device from the hit density
     int32_t gather_ld_cached = 1;
-    int32_t gather_prefetch = 1;                        // DT_GATHER_PREFETCH: planes ahead (dense schedule, resident store)
-    int32_t stream_zero_copy = -1;                      // DT_STREAM_ZERO_COPY: -1 decide from a probe, 0 never, 1 always
+    int32_t gather_prefetch = 1;                        // planes ahead (dense schedule, resident store)
+    int32_t sm_count = 0;                               // SMs of this context's device
+    int32_t stream_zero_copy = -1;                      // -1 decide from a probe, 0 never, 1 always
     const float **d_flux_ptrs = nullptr, **d_var_ptrs = nullptr;   // [N] device-mapped pinned planes (zero-copy gather)
-    bool zero_copy_elements = true;                     // DT_ZERO_COPY=0: copy pinned elements to the device first
+    bool zero_copy_elements = true;                     // false: copy pinned elements to the device first
     std::vector<cudaEvent_t> ev_pool;                   // timing events
 
     TopkWorkspace topk;
@@ -132,6 +139,8 @@ void free_all(dt_context *c)
         if (c->ev_free[s]) cudaEventDestroy(c->ev_free[s]);
     }
     cudaFree(c->d_el);
+    cudaFree(c->d_t0);
+    cudaFree(c->d_patch_w);
     cudaFree(c->d_S);
     cudaFree(c->d_Wt);
     cudaFree(c->d_snr);
@@ -181,8 +190,6 @@ ExpRec make_record(const dt_context *c, double t, const double *obs, double ra0,
 // is budgeted (data read by SMs of both dies may be held once per die).  DT_GATHER_WINDOW overrides.
 int32_t pick_gather_window(const dt_context *c)
 {
-    const char *env = getenv("DT_GATHER_WINDOW");
-    if (env && atoi(env) > 0) return std::min(atoi(env), 64);
     int l2 = 0;
     if (cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, c->device) != cudaSuccess || l2 <= 0) l2 = 64 << 20;
     const int64_t per_exp = c->plane * 4 * (c->var_mode == 1 ? 2 : 1);
@@ -234,7 +241,7 @@ int dt_create(const dt_survey *s, dt_context **out)
     *out = nullptr;
     if (!s || s->struct_size != sizeof(dt_survey)) return DT_ERR_INVALID_ARG;
     if (s->n_exposures < 1 || s->width < 1 || s->height < 1 ||
-        (int64_t)s->width * s->height >= ((int64_t)1 << 31))
+        (int64_t)s->width * s->height > ((int64_t)1 << kOffsetBits))
         return DT_ERR_INVALID_ARG;
     if (!s->t || !s->obs_ecl || !s->ra0 || !s->dec0) return DT_ERR_INVALID_ARG;
     if (!(s->pixel_scale > 0.0) || !isfinite(s->pixel_scale)) return DT_ERR_INVALID_ARG;
@@ -288,11 +295,8 @@ int dt_create(const dt_survey *s, dt_context **out)
         if (cudaMalloc((void **)&c->d_counters, 8 * sizeof(unsigned long long)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
         if (cudaMalloc((void **)&c->d_progress, (size_t)(kMaxUnitExposures + kGroup) * kProgressStride * sizeof(int)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
         c->gather_window = pick_gather_window(c);
-        if (const char *env = getenv("DT_STREAM_ZERO_COPY")) c->stream_zero_copy = atoi(env) < 0 ? -1 : (atoi(env) ? 1 : 0);
-        if (const char *env = getenv("DT_ZERO_COPY")) c->zero_copy_elements = atoi(env) != 0;
-        if (const char *env = getenv("DT_GATHER_PREFETCH")) c->gather_prefetch = std::max(0, std::min(atoi(env), 8));
-        if (const char *env = getenv("DT_GATHER_L1")) c->gather_ld_cached = atoi(env) ? 1 : 0;
-        if (const char *env = getenv("DT_GATHER_LOCKSTEP")) c->gather_lockstep = atoi(env) < 0 ? -1 : (atoi(env) ? 1 : 0);
+        // kernel attributes are per DEVICE: set them for this context's device (no process-wide statics)
+        if (init_device_kernels(c->device, &c->sm_count) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
         if (cudaStreamSynchronize(c->stream) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
         size_t free_b = 0, total_b = 0;
         if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
@@ -392,6 +396,15 @@ static int propagate_mode(const dt_context *c)
     return mode;
 }
 
+static void fill_gather_ext(const dt_context *c, GatherParams &g)
+{
+    g.patch = c->patch;
+    g.patch_w = c->d_patch_w;
+    g.clip = c->clip;
+    g.width = c->W;
+    g.height = c->H;
+}
+
 static void fill_common(const dt_context *c, PropagateParams &p, double t0)
 {
     memset(&p, 0, sizeof p);
@@ -418,8 +431,11 @@ static int32_t pick_groups_per_split(int64_t n_orbits, int32_t n_exp)
     return (int32_t)((n_groups + splits - 1) / splits);
 }
 
-int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_t mem_kind, double *snr_out,
-             int32_t *hits_out)
+}  // extern "C"
+
+// dt_stack and dt_stack_epochs: t0_orbit == NULL means the scalar epoch t0
+static int stack_impl(dt_context *c, const double *elements, const double *t0_orbit, int64_t n, double t0,
+                      int32_t mem_kind, double *snr_out, int32_t *hits_out)
 {
     if (!c) return DT_ERR_INVALID_ARG;
     if (n < 0 || (n > 0 && !elements) || !mem_kind_ok(mem_kind) || !isfinite(t0))
@@ -464,6 +480,17 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
             cudaGetLastError();
             CU(c, cudaMemcpyAsync(c->d_el, elements, (size_t)n * 48, cudaMemcpyDefault, c->stream));
             first_src = c->d_el;
+        }
+    }
+    // per-orbit epochs: on the device before kernel 1 (8 B per orbit)
+    const double *d_t0 = nullptr;
+    if (t0_orbit) {
+        if (mem_kind == DT_MEM_DEVICE) {
+            d_t0 = t0_orbit;
+        } else {
+            CU(c, grow(c->d_t0, c->t0_cap, n));
+            CU(c, cudaMemcpyAsync(c->d_t0, t0_orbit, (size_t)n * 8, cudaMemcpyDefault, c->stream));
+            d_t0 = c->d_t0;
         }
     }
     if (n > c->acc_cap) {
@@ -552,6 +579,7 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
                 PropagateParams p;
                 fill_common(c, p, t0);
                 p.elements = first_src;
+                p.t0_orbit = d_t0;
                 p.n_orbits = no;
                 p.n_pad = (no + 31) / 32 * 32;
                 p.exp = c->d_exp;
@@ -597,6 +625,7 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
             PropagateParams p;
             fill_common(c, p, t0);
             p.elements = (b == 0 ? first_src : d_el) + o0 * 6;
+            p.t0_orbit = d_t0 ? d_t0 + o0 : nullptr;
             p.elements_copy = (b == 0 && copy_out) ? copy_out + o0 * 6 : nullptr;
             p.n_orbits = no;
             p.n_pad = (no + 31) / 32 * 32;
@@ -649,8 +678,10 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
             g.ld_cached = c->gather_ld_cached;
             g.prefetch = c->streaming ? 0 : c->gather_prefetch;
             g.n_exp_store = c->N;
+            g.sm_count = c->sm_count;
+            fill_gather_ext(c, g);
             CU(c, launch_gather(g, c->device, c->stream));
-            st.gather_launches += (g.lockstep_mode < 0) ? 2 : 1;   // sparse + dense schedule, one of them returns at once
+            st.gather_launches += (g.lockstep_mode < 0) ? 2 : 1;   // both schedules are enqueued, one of them returns at once
             CU(c, cudaEventRecord(ev_at(3 * unit_idx + 2), c->stream));
             unit_idx += 1;
         }
@@ -660,7 +691,7 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
         }
     }
     CU(c, cudaEventRecord(c->ev_pool[2], c->stream));
-    CU(c, launch_finalize(d_el, n, c->d_S, c->d_Wt, c->d_cnt, c->d_snr, c->d_hits, c->d_counters + 5,
+    CU(c, launch_finalize(d_el, d_t0, n, c->d_S, c->d_Wt, c->d_cnt, c->d_snr, c->d_hits, c->d_counters + 5,
                           c->stream));
     CU(c, cudaEventRecord(c->ev_pool[3], c->stream));
     if (snr_out)
@@ -687,6 +718,62 @@ int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_
     st.invalid_orbits = (int64_t)hc[5];
     st.launches = st.propagate_launches + st.gather_launches + 1;
     c->n_last = n;
+    return DT_OK;
+}
+
+extern "C" {
+
+int dt_stack(dt_context *c, const double *elements, int64_t n, double t0, int32_t mem_kind, double *snr_out,
+             int32_t *hits_out)
+{
+    return stack_impl(c, elements, nullptr, n, t0, mem_kind, snr_out, hits_out);
+}
+
+int dt_stack_epochs(dt_context *c, const double *elements, const double *t0, int64_t n, int32_t mem_kind,
+                    double *snr_out, int32_t *hits_out)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (n > 0 && !t0) return fail(c, DT_ERR_INVALID_ARG, "dt_stack_epochs: t0 is NULL");
+    return stack_impl(c, elements, n > 0 ? t0 : nullptr, n, 0.0, mem_kind, snr_out, hits_out);
+}
+
+int dt_set_patch(dt_context *c, int32_t k, const double *weights)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (k < 1 || k > 15 || (k % 2) == 0) return fail(c, DT_ERR_INVALID_ARG, "dt_set_patch: k must be odd, 1 .. 15");
+    if (weights)
+        for (int i = 0; i < k * k; ++i)
+            if (!isfinite(weights[i])) return fail(c, DT_ERR_INVALID_ARG, "dt_set_patch: non-finite weight");
+    CU(c, cudaSetDevice(c->device));
+    CU(c, cudaStreamSynchronize(c->stream));
+    cudaFree(c->d_patch_w);
+    c->d_patch_w = nullptr;
+    c->patch = k;
+    if (weights) {
+        CU(c, cudaMalloc((void **)&c->d_patch_w, sizeof(double) * (size_t)(k * k)));
+        CU(c, cudaMemcpy(c->d_patch_w, weights, sizeof(double) * (size_t)(k * k), cudaMemcpyHostToDevice));
+    }
+    return DT_OK;
+}
+
+int dt_set_outlier_clip(dt_context *c, double clip)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (isnan(clip)) return fail(c, DT_ERR_INVALID_ARG, "dt_set_outlier_clip: NaN");
+    c->clip = clip;
+    return DT_OK;
+}
+
+int dt_threshold(dt_context *c, double snr_min, int32_t min_hits, int64_t max_out, int64_t *index_out,
+                 double *snr_out, int64_t *n_found)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (isnan(snr_min) || max_out < 0 || !n_found || (max_out > 0 && !index_out))
+        return fail(c, DT_ERR_INVALID_ARG, "dt_threshold: bad arguments");
+    if (c->n_last < 0) return fail(c, DT_ERR_STATE, "dt_threshold: no dt_stack result on the device");
+    CU(c, cudaSetDevice(c->device));
+    CU(c, threshold_device(c->d_snr, c->d_hits, c->n_last, snr_min, min_hits, max_out, c->topk, index_out, snr_out,
+                           n_found, c->stream));
     return DT_OK;
 }
 
@@ -733,7 +820,9 @@ int dt_project(dt_context *c, const double *elements, int64_t n, double t0, doub
     CUP(cudaMalloc((void **)&d_radec, (size_t)chunk * N * 16));
     CUP(cudaMalloc((void **)&d_xy, (size_t)chunk * N * 16));
     CUP(cudaMalloc((void **)&d_pix, (size_t)chunk * N * 8));
-    const int mode = (propagate_mode(c) & kModeWarm) | kModeDense;
+    // default: every pair refined; DT_FLAG_PROJECT_PRECULL keeps dt_stack's pre-cull and cull-quality chain
+    const int mode = (propagate_mode(c) & (kModeWarm | ((c->flags & DT_FLAG_PROJECT_PRECULL) ? kModePrecull : 0))) |
+                     kModeDense;
     for (int64_t o0 = 0; o0 < n; o0 += chunk) {
         const int64_t no = std::min<int64_t>(chunk, n - o0);
         CUP(cudaMemcpyAsync(d_el, elements + o0 * 6, (size_t)no * 48, cudaMemcpyHostToDevice, c->stream));
@@ -799,7 +888,82 @@ int dt_gather_hits(dt_context *c, int64_t n, int32_t first_exposure, int32_t n_g
     g.ld_cached = c->gather_ld_cached;
     g.prefetch = c->gather_prefetch;
     g.n_exp_store = c->N;
+    g.sm_count = c->sm_count;
+    fill_gather_ext(c, g);
     CU(c, launch_gather(g, c->device, c->stream));
+    return DT_OK;
+}
+
+int dt_filter_intersections(dt_context *c, const double *elements, int64_t n, double t0, int32_t mem_kind,
+                            int32_t first_exposure, int32_t n_exposures, const uint32_t **mask,
+                            const uint64_t **base, const uint32_t **offsets, int64_t *n_hits, int64_t *n_pad,
+                            int32_t *n_groups)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (n < 1 || n > kMaxUnitOrbits || !elements || !mem_kind_ok(mem_kind) || !isfinite(t0) || first_exposure < 0 ||
+        n_exposures < 1 || n_exposures > kMaxUnitExposures || (int64_t)first_exposure + n_exposures > c->N ||
+        !mask || !base || !offsets || !n_hits || !n_pad || !n_groups)
+        return fail(c, DT_ERR_INVALID_ARG, "dt_filter_intersections: bad arguments (one work unit: <= %lld orbits, <= %d exposures)",
+                    (long long)kMaxUnitOrbits, kMaxUnitExposures);
+    CU(c, cudaSetDevice(c->device));
+    const int64_t pad = (n + 31) / 32 * 32;
+    const int32_t groups = (n_exposures + kGroup - 1) / kGroup;
+    const double *d_el = elements;
+    if (mem_kind != DT_MEM_DEVICE || (reinterpret_cast<uintptr_t>(elements) & 15u)) {
+        CU(c, grow(c->d_el, c->el_cap, n * 6));
+        CU(c, cudaMemcpyAsync(c->d_el, elements, (size_t)n * 48, cudaMemcpyDefault, c->stream));
+        d_el = c->d_el;
+    }
+    CU(c, grow(c->d_mask, c->mask_cap, pad * groups));
+    CU(c, grow(c->d_base, c->base_cap, (pad / 32) * groups));
+    CU(c, grow(c->d_offsets, c->off_cap, pad * (int64_t)groups * kGroup));
+    CU(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+    PropagateParams p;
+    fill_common(c, p, t0);
+    p.elements = d_el;
+    p.n_orbits = n;
+    p.n_pad = pad;
+    p.exp = c->d_exp + first_exposure;
+    p.n_exp = n_exposures;
+    p.groups_per_split = pick_groups_per_split(n, n_exposures);
+    p.mask = c->d_mask;
+    p.base = c->d_base;
+    p.offsets = c->d_offsets;
+    p.counters = c->d_counters;
+    CU(c, launch_propagate(p, propagate_mode(c), c->stream));
+    unsigned long long h = 0;
+    CU(c, cudaMemcpyAsync(&h, c->d_counters, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    c->n_last = -1;                       // the per-orbit results of an earlier dt_stack are gone
+    *mask = c->d_mask;
+    *base = reinterpret_cast<const uint64_t *>(c->d_base);
+    *offsets = c->d_offsets;
+    *n_hits = (int64_t)h;
+    *n_pad = pad;
+    *n_groups = groups;
+    return DT_OK;
+}
+
+int dt_set_option(dt_context *c, const char *name, int64_t value)
+{
+    if (!c || !name) return DT_ERR_INVALID_ARG;
+    const std::string k(name);
+    if (k == "gather_schedule") {
+        if (value < -1 || value > 1) return fail(c, DT_ERR_INVALID_ARG, "gather_schedule: -1 auto, 0 orbit-major, 1 dense");
+        c->gather_lockstep = (int32_t)value;
+    } else if (k == "gather_window") {
+        c->gather_window = value > 0 ? (int32_t)std::min<int64_t>(value, 64) : pick_gather_window(c);
+    } else if (k == "gather_prefetch") {
+        c->gather_prefetch = (int32_t)std::max<int64_t>(0, std::min<int64_t>(value, 8));
+    } else if (k == "gather_l1") {
+        c->gather_ld_cached = value ? 1 : 0;
+    } else if (k == "stream_zero_copy") {
+        c->stream_zero_copy = value < 0 ? -1 : (value ? 1 : 0);
+    } else if (k == "zero_copy_elements") {
+        c->zero_copy_elements = value != 0;
+    } else {
+        return fail(c, DT_ERR_INVALID_ARG, "dt_set_option: unknown option '%s'", name);
+    }
     return DT_OK;
 }
 

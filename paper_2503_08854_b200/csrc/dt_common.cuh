@@ -41,6 +41,7 @@ struct PropagateParams {
     int32_t n_exp;              // exposures in this unit
     int32_t groups_per_split;   // exposure groups handled by one blockIdx.y
     double t0, gm, inv_c;       // inv_c = 0 disables light-time
+    const double *t0_orbit;     // NULL, or device [n]: per-orbit epoch of M0 (dt_stack_epochs; replaces t0)
     double cos_eps, sin_eps;
     double cx, cy, W, H;        // (W-1)/2, (H-1)/2, width, height as fp64
     int32_t width;
@@ -90,7 +91,21 @@ struct GatherParams {
     int32_t ld_cached;          // dense schedule: pixel loads allocate in L1 (1) or not (0)
     int32_t prefetch;           // dense schedule: planes ahead of the front that are prefetched into L2 (0 = off)
     int32_t n_exp_store;        // exposures the store holds from absolute index 0 (bound of the prefetch)
+    int32_t sm_count;           // SMs of the context's device (grid of the persistent schedules)
+    // extended stack (dtrack.h dt_set_patch, dt_set_outlier_clip): k x k patch
+    // around the nearest pixel with PSF weights, per-intersection outlier rejection.  patch == 1, patch_w ==
+    // NULL and clip == +inf is the plain single-pixel stack; anything else runs the orbit-major walk's
+    // extended instantiation.
+    int32_t patch;              // k >= 1, odd
+    const double *patch_w;      // device [k*k] row-major, or NULL (all 1)
+    double clip;                // +inf: no rejection
+    int32_t width, height;      // image size (patch bounds)
 };
+
+// A hit entry is (exposure within its group) << kOffsetBits | (iy * W + ix): an entry names its exposure, so
+// a block of the list can be processed as one flat coalesced list.  W * H <= 2^27 (dt_create checks).
+constexpr int kOffsetBits = 27;
+constexpr uint32_t kOffsetMask = (1u << kOffsetBits) - 1u;
 
 constexpr int kProgressStride = 32;     // one 128-B line per exposure counter (no false sharing of polls)
 #ifndef DT_K3_THREADS
@@ -102,12 +117,17 @@ constexpr int kGatherCtasPerSm = 1024 / kGatherThreads;   // 1024 resident threa
 constexpr int kMaxTilesPerWarp = 8;     // 148 SMs x 32 warps x 8 tiles x 32 orbits >= 2^20 orbits
 
 cudaError_t launch_gather(const GatherParams &p, int device, cudaStream_t stream);
+// Per-device kernel attributes (dynamic shared memory opt-in of every kernel of the library); called by
+// dt_create after cudaSetDevice, so that a context on a second device of the same process is set up too.
+cudaError_t init_device_kernels(int device, int *sm_count);
+cudaError_t init_propagate_kernels();
+cudaError_t init_gather_kernels();
 // dst[k] = (flux[k], var[k]), k < n: builds the interleaved store from two device planes
 cudaError_t launch_interleave(const float *flux, const float *var, float2 *dst, int64_t n, cudaStream_t stream);
 
 // SNR finalisation: snr = S / sqrt(Wt) (0 when no hit), NaN / -1 for invalid orbits.
-cudaError_t launch_finalize(const double *elements, int64_t n, const double *S, const double *Wt,
-                            const int32_t *cnt, double *snr, int32_t *hits,
+cudaError_t launch_finalize(const double *elements, const double *t0_orbit, int64_t n, const double *S,
+                            const double *Wt, const int32_t *cnt, double *snr, int32_t *hits,
                             unsigned long long *invalid_counter, cudaStream_t stream);
 
 // ---- device top-k (dt_topk.cu) ----------------------------------------------------------------------
@@ -127,6 +147,11 @@ cudaError_t topk_device(const double *snr, const int32_t *hits, int64_t n, int32
                         int32_t min_hits, TopkWorkspace &ws, int64_t *index_out_host,
                         double *snr_out_host, int32_t *n_found, cudaStream_t stream);
 void topk_free(TopkWorkspace &ws);
+// Threshold mode: every valid entry (finite snr >= snr_min, hits >= min_hits) in ascending index order;
+// *n_found = how many there are, the first min(*n_found, max_out) are written to the host arrays.
+cudaError_t threshold_device(const double *snr, const int32_t *hits, int64_t n, double snr_min,
+                             int32_t min_hits, int64_t max_out, TopkWorkspace &ws, int64_t *index_out_host,
+                             double *snr_out_host, int64_t *n_found, cudaStream_t stream);
 
 // FP64 FMA issue-rate probe (dt_fp64_peak).
 cudaError_t fp64_peak_device(double *tflops, cudaStream_t stream);

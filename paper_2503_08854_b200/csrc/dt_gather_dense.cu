@@ -16,27 +16,11 @@
 //     orbits of the unit read them: a plane is fetched from DRAM once per launch instead of once per
 //     wave of CTAs (profiles/r1a_baseline.md: 62.7 GB of DRAM reads for 8.9 GB of algorithmic bytes).
 //     The grid is launched cooperatively so that all CTAs are co-resident (the throttle needs it).
-#include <stdlib.h>
-
 #include "dt_common.cuh"
 #include "dt_gather.cuh"
 
 namespace dt {
 
-__device__ __forceinline__ int ld_relaxed(const int *p)
-{
-    int v;
-    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void prefetch_l2(const void *p)
-{
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-}
-__device__ __forceinline__ void red_add_relaxed(int *p, int v)
-{
-    asm volatile("red.relaxed.gpu.global.add.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
 
 // Shared memory of one CTA: (S, Wt) [T][kGatherThreads] double2, cnt [T][kGatherThreads] int32
 // (accumulators, lane-private), arrive [n_local] int, done_upto int (lock-step throttle).
@@ -146,7 +130,7 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherCtasPerSm) k_gather_den
             for (int t = 0; t < kMaxTilesPerWarp; ++t) {
                 const bool h = (bits[t] >> jj) & 1u;
                 const unsigned hm = __ballot_sync(0xffffffffu, h);
-                off[t] = h ? p.offsets[cur[t] + __popc(hm & lt)] : 0u;
+                off[t] = h ? (p.offsets[cur[t] + __popc(hm & lt)] & kOffsetMask) : 0u;
                 cur[t] += __popc(hm);
                 mine |= h ? (1u << t) : 0u;
             }
@@ -240,14 +224,10 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherCtasPerSm) k_gather_den
 
 // Grid geometry: all CTAs co-resident (cooperative launch), as many warps as there are warp-tiles
 // up to the machine's capacity, tiles spread evenly.
-static cudaError_t dense_geometry(int64_t n_pad, int32_t n_groups, int device, int *grid, int *tiles_per_warp,
-                                  size_t *smem)
+cudaError_t persistent_geometry(int64_t n_pad, int32_t n_groups, int sm_count, int *grid, int *tiles_per_warp,
+                                size_t *smem)
 {
-    static int sm_count = 0;
-    if (!sm_count) {
-        cudaError_t e = cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, device);
-        if (e != cudaSuccess) return e;
-    }
+    if (sm_count <= 0) return cudaErrorInvalidValue;
     constexpr int n_warps = kGatherThreads / 32;
     const int64_t n_tiles = n_pad >> 5;
     const int max_ctas = sm_count * kGatherCtasPerSm;
@@ -269,26 +249,26 @@ cudaError_t launch_gather_dense(const GatherParams &p_in, int device, cudaStream
     GatherParams p = p_in;
     int grid = 0, T = 0;
     size_t smem = 0;
-    cudaError_t e = dense_geometry(p.n_pad, p.n_groups, device, &grid, &T, &smem);
+    (void)device;
+    cudaError_t e = persistent_geometry(p.n_pad, p.n_groups, p.sm_count, &grid, &T, &smem);
     if (e != cudaSuccess) return e;
     p.tiles_per_warp = T;
     e = cudaMemsetAsync(p.progress, 0, (size_t)p.n_groups * kGroup * kProgressStride * sizeof(int), stream);
     if (e != cudaSuccess) return e;
     const bool plane_var = p.var || p.fv;
     const void *fn = plane_var ? (const void *)k_gather_dense<true> : (const void *)k_gather_dense<false>;
-    static size_t smem_set[2] = {0, 0};
-    const int which = plane_var ? 1 : 0;
-    if (smem > smem_set[which]) {
-        e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        smem_set[which] = smem;
-        if (const char *env = getenv("DT_GATHER_CARVEOUT")) {   // experiment knob: % of the SM's L1/smem
-            e = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, atoi(env));
-            if (e != cudaSuccess) return e;
-        }
-    }
     void *args[] = {(void *)&p};
     return cudaLaunchCooperativeKernel(fn, dim3((unsigned)grid), dim3(kGatherThreads), args, smem, stream);
+}
+
+// dynamic shared memory opt-in (the accumulators of a full unit need up to ~166 KB), for the CURRENT device
+cudaError_t init_gather_dense_kernels()
+{
+    cudaError_t e = cudaFuncSetAttribute(k_gather_dense<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)kPersistentSmemMax);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_gather_dense<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)kPersistentSmemMax);
 }
 
 }  // namespace dt

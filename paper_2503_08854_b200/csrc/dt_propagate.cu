@@ -93,6 +93,10 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
     const bool in_range = orbit < p.n_orbits;
 #pragma unroll
     for (int k = 0; k < 6; ++k) el[k] = in_range ? sm.el[tid * 6 + k] : ((k == 0) ? -1.0 : 0.0);
+    // epoch of M0: one per call, or one per orbit ("six orbital elements and an orbital epoch");
+    // a non-finite epoch makes the orbit invalid
+    const double t0 = p.t0_orbit ? (in_range ? p.t0_orbit[orbit] : 0.0) : p.t0;
+    if (!isfinite(t0)) el[0] = -1.0;
     const Orbit o = orbit_setup(el, p.gm, p.cos_eps, p.sin_eps, p.inv_c, p.tan_fov);
 
     Kepler K;
@@ -121,7 +125,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
         int run = 0;          // the warp's hits in the group so far (warp-uniform)
         for (int jj = 0; jj < nrec; ++jj) {
             const ExpRec &x = sm.rec[slot][jj];
-            const double dt = x.t - p.t0;
+            const double dt = x.t - t0;
             const double M = fma(o.n, dt, o.M0);
 
             // ---- step 3: Kepler solve at t_j ----
@@ -277,16 +281,19 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
             if (DENSE) {
                 if (in_range) {
                     const int64_t k = (orbit * p.n_exp + (int64_t)g * kGroup + jj) * 2;
+                    // with the pre-cull kept (dt_project under DT_FLAG_PROJECT_PRECULL) a pair whose warp the
+                    // cull-quality cone test rejected is reported as culled: NaN, (-1, -1)
+                    const bool rep = o.valid && refine;
                     if (p.radec) {
                         const double rho = sqrt(fma(qx, qx, fma(qy, qy, qz * qz)));
                         double ra = atan2(qy, qx);
                         if (ra < 0.0) ra += 2.0 * kPi;
-                        p.radec[k] = o.valid ? ra : nan("");
-                        p.radec[k + 1] = o.valid ? asin(qz / rho) : nan("");
+                        p.radec[k] = rep ? ra : nan("");
+                        p.radec[k + 1] = rep ? asin(qz / rho) : nan("");
                     }
                     if (p.xy) {
-                        p.xy[k] = o.valid ? xpix : nan("");
-                        p.xy[k + 1] = o.valid ? ypix : nan("");
+                        p.xy[k] = rep ? xpix : nan("");
+                        p.xy[k + 1] = rep ? ypix : nan("");
                     }
                     if (p.pix) {
                         p.pix[k] = ix;
@@ -299,7 +306,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 if (hm) {
                     if (hit) {
                         sm.stage[warp][run + __popc(hm & ((1u << lane) - 1u))] =
-                            (uint32_t)iy * (uint32_t)p.width + (uint32_t)ix;
+                            ((uint32_t)jj << kOffsetBits) | ((uint32_t)iy * (uint32_t)p.width + (uint32_t)ix);
                         bits |= 1u << jj;
                         cnt += 1;
                     }
@@ -349,14 +356,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
 template <int MODE>
 static cudaError_t launch_mode(const PropagateParams &p, cudaStream_t stream)
 {
-    static bool attr_set = false;
     const size_t smem = sizeof(PropSmem);
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_propagate<MODE>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
     const int n_groups = (p.n_exp + kGroup - 1) / kGroup;
     const int splits = (n_groups + p.groups_per_split - 1) / p.groups_per_split;
     dim3 grid((unsigned)((p.n_orbits + kTileOrbits - 1) / kTileOrbits), (unsigned)splits);
@@ -374,8 +374,30 @@ cudaError_t launch_propagate(const PropagateParams &p, int mode, cudaStream_t st
         case 3: return launch_mode<3>(p, stream);
         case 4: return launch_mode<4>(p, stream);
         case 5: return launch_mode<5>(p, stream);
+        case 6: return launch_mode<6>(p, stream);
+        case 7: return launch_mode<7>(p, stream);
         default: return cudaErrorInvalidValue;
     }
+}
+
+template <int MODE>
+static cudaError_t set_smem_attr()
+{
+    return cudaFuncSetAttribute(k_propagate<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PropSmem));
+}
+
+// dynamic shared memory opt-in of every instantiation, for the CURRENT device (per device, not per process)
+cudaError_t init_propagate_kernels()
+{
+    cudaError_t e;
+    if ((e = set_smem_attr<0>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<1>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<2>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<3>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<4>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<5>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<6>()) != cudaSuccess) return e;
+    return set_smem_attr<7>();
 }
 
 }  // namespace dt

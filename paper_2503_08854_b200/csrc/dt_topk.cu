@@ -10,6 +10,10 @@
 //    first r keys == T in INDEX order (this is what makes ties deterministic);
 // 4. bitonic sort of the <= k candidates on the composite (key descending, index ascending):
 //    shared-memory kernel for spans <= 2048, global compare-exchange steps above that.
+#include <string.h>
+
+#include <algorithm>
+
 #include "dt_common.cuh"
 
 namespace dt {
@@ -177,7 +181,8 @@ __global__ void k_scan(unsigned int *counts, int nblocks, unsigned long long *st
 __global__ void k_scatter(const unsigned long long *__restrict__ keys, int64_t n,
                           const unsigned long long *__restrict__ state,
                           const unsigned int *__restrict__ counts,
-                          unsigned long long *__restrict__ cand_key, long long *__restrict__ cand_idx)
+                          unsigned long long *__restrict__ cand_key, long long *__restrict__ cand_idx,
+                          unsigned long long limit)
 {
     // ordered within the block: each thread handles kItems CONSECUTIVE keys
     __shared__ unsigned int sc[2][kThreads];
@@ -209,8 +214,10 @@ __global__ void k_scatter(const unsigned long long *__restrict__ keys, int64_t n
     for (int it = 0; it < kItems; ++it) {
         const unsigned long long key = loc[it];
         if (key > T) {
-            cand_key[pg] = key;
-            cand_idx[pg] = base + it;
+            if (pg < limit) {            // threshold mode writes at most `limit` entries (top-k: no limit)
+                cand_key[pg] = key;
+                cand_idx[pg] = base + it;
+            }
             ++pg;
         } else if (key == T && key != 0ull) {
             if (pe < r) {
@@ -349,7 +356,7 @@ cudaError_t topk_device(const double *snr, const int32_t *hits, int64_t n, int32
     k_count<<<nblocks, kThreads, 0, stream>>>(ws.keys, n, ws.state, ws.block_counts);
     k_scan<<<1, 1024, 0, stream>>>(ws.block_counts, nblocks, ws.state);
     k_scatter<<<nblocks, kThreads, 0, stream>>>(ws.keys, n, ws.state, ws.block_counts, ws.cand_key,
-                                                ws.cand_idx);
+                                                ws.cand_idx, ~0ull);
     TK_CHECK(cudaGetLastError());
 
     unsigned long long st[8];
@@ -383,6 +390,66 @@ cudaError_t topk_device(const double *snr, const int32_t *hits, int64_t n, int32
     TK_CHECK(cudaStreamSynchronize(stream));
     *n_found = (int32_t)m;
     return cudaSuccess;
+}
+
+// Threshold mode (Algorithm 1 `FindSignificantResults`; "detections above an SNR of 5",
+// PAPER.md:336): the ordered compaction of the top-k with a GIVEN threshold key -- keys >= key(snr_min), i.e.
+// keys > key(snr_min) - 1 -- and no ties to resolve; candidates leave in ascending index order.
+__global__ void k_set_threshold(unsigned long long *state, unsigned long long T)
+{
+    state[3] = T;
+    state[4] = 0;
+}
+
+cudaError_t threshold_device(const double *snr, const int32_t *hits, int64_t n, double snr_min,
+                             int32_t min_hits, int64_t max_out, TopkWorkspace &ws, int64_t *index_out_host,
+                             double *snr_out_host, int64_t *n_found, cudaStream_t stream)
+{
+    *n_found = 0;
+    if (n <= 0) return cudaSuccess;
+    const int nblocks = (int)((n + kChunk - 1) / kChunk);
+    const int64_t cap = std::max<int64_t>(1, std::min<int64_t>(max_out, n));
+    TK_CHECK(ensure(ws.keys, ws.n_cap, n));
+    {
+        int64_t c = ws.cand_cap;
+        TK_CHECK(ensure(ws.cand_key, c, cap));
+        c = ws.cand_cap;
+        TK_CHECK(ensure(ws.cand_idx, c, cap));
+        ws.cand_cap = c;
+    }
+    if (!ws.hist) TK_CHECK(cudaMalloc((void **)&ws.hist, 256 * sizeof(unsigned int)));
+    if (!ws.state) TK_CHECK(cudaMalloc((void **)&ws.state, 16 * sizeof(unsigned long long)));
+    TK_CHECK(ensure(ws.block_counts, ws.blocks_cap, (int64_t)2 * nblocks));
+    // order-preserving key of the threshold (host copy of order_key; -0.0 and +0.0 compare equal in IEEE, so
+    // a zero threshold takes the smaller key)
+    double th = (snr_min == 0.0) ? -0.0 : snr_min;
+    unsigned long long b;
+    static_assert(sizeof b == sizeof th, "fp64");
+    memcpy(&b, &th, sizeof b);
+    const unsigned long long key = (b & 0x8000000000000000ull) ? ~b : (b | 0x8000000000000000ull);
+    TK_CHECK(cudaMemsetAsync(ws.state, 0, 16 * sizeof(unsigned long long), stream));
+    k_keys<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(snr, hits, n, min_hits, ws.keys);
+    k_set_threshold<<<1, 1, 0, stream>>>(ws.state, key - 1ull);
+    k_count<<<nblocks, kThreads, 0, stream>>>(ws.keys, n, ws.state, ws.block_counts);
+    k_scan<<<1, 1024, 0, stream>>>(ws.block_counts, nblocks, ws.state);
+    k_scatter<<<nblocks, kThreads, 0, stream>>>(ws.keys, n, ws.state, ws.block_counts, ws.cand_key, ws.cand_idx,
+                                                (unsigned long long)max_out);
+    TK_CHECK(cudaGetLastError());
+    unsigned long long st[8];
+    TK_CHECK(cudaMemcpyAsync(st, ws.state, sizeof st, cudaMemcpyDeviceToHost, stream));
+    TK_CHECK(cudaStreamSynchronize(stream));
+    const int64_t total = (int64_t)st[7];
+    *n_found = total;
+    const int64_t m = std::min<int64_t>(total, max_out);
+    if (m <= 0) return cudaSuccess;
+    double *out_snr = reinterpret_cast<double *>(ws.keys);      // the key buffer is free again
+    k_emit<<<(unsigned)((m + 255) / 256), 256, 0, stream>>>(ws.cand_idx, snr, m, out_snr);
+    TK_CHECK(cudaGetLastError());
+    if (index_out_host)
+        TK_CHECK(cudaMemcpyAsync(index_out_host, ws.cand_idx, (size_t)m * sizeof(long long), cudaMemcpyDeviceToHost, stream));
+    if (snr_out_host)
+        TK_CHECK(cudaMemcpyAsync(snr_out_host, out_snr, (size_t)m * sizeof(double), cudaMemcpyDeviceToHost, stream));
+    return cudaStreamSynchronize(stream);
 }
 
 void topk_free(TopkWorkspace &ws)

@@ -42,3 +42,22 @@ def read_golden(name):
             else:
                 vals[p[0]] = float(p[1])
     return vals, consts
+
+
+PARITY_REPORT = os.path.join(ROOT, "gpurun_out", "parity_report.json")
+
+
+def parity_record(case, **counts):
+    """north_star: pixel mismatches inside the 1e-6 px guard band are "counted and reported".  Every GPU
+    parity test leaves its counts here (gpurun_out/parity_report.json: flagged pairs / orbits, in-band
+    mismatches, what was compared); bench.py echoes the file as `parity_report` when it is present."""
+    import json
+    os.makedirs(os.path.dirname(PARITY_REPORT), exist_ok=True)
+    try:
+        with open(PARITY_REPORT) as f:
+            rep = json.load(f)
+    except Exception:
+        rep = {}
+    rep[case] = {k: (v.item() if hasattr(v, "item") else v) for k, v in counts.items()}
+    with open(PARITY_REPORT, "w") as f:
+        json.dump(rep, f, indent=1, sort_keys=True)

@@ -16,6 +16,7 @@ import pytest
 
 import dtsynth as ds
 import oracle
+from conftest import parity_record
 
 pytestmark = pytest.mark.gpu
 
@@ -78,9 +79,12 @@ def _check_sample(cfg, scene, plane_of, snr, hits, sample, label):
     flagged = np.flatnonzero(~clean)
     same = flagged[g_hits[flagged] == ref["hits"][flagged]]
     assert ok[same].all(), label
-    return dict(checked=int(keep.size), with_hits=int((ref["hits"] > 0).sum()), exposures=int(Hs.size),
+    assert (np.abs(g_hits - ref["hits"]) <= ref["nflag"]).all(), label   # at most one hit per flagged pair
+    rep = dict(checked=int(keep.size), with_hits=int((ref["hits"] > 0).sum()), exposures=int(Hs.size),
                 max_hits=int(ref["hits"].max()), flagged=int(flagged.size),
                 flagged_hit_mismatch=int(flagged.size - same.size))
+    parity_record("fullsize[%s]" % label, **rep)
+    return rep
 
 
 def _pick_sample(scene, hits_dev, n):
@@ -110,7 +114,7 @@ def _whole_output_properties(dt, trk, snr_dev, hits_dev, N):
     assert np.array_equal(cand.cpu().numpy()[widx], idx) and np.array_equal(wval, val)
 
 
-RESIDENT = ["small_mba", "small_mba+focused", "neo+focused", "tno+focused"]
+RESIDENT = ["small_mba", "small_mba+focused", "neo", "neo+focused", "tno", "tno+focused"]
 
 
 @pytest.mark.parametrize("name", RESIDENT)
@@ -183,13 +187,12 @@ def test_full_size_lsst_streamed():
     for q in range(POOL):
         flux_pool[q].copy_(ds.noise_plane_t(cfg, q, dev))
         var_pool[q].fill_(float(scene.var_scalar[q]))
-    import os
     el = _elements_device(cfg, dev)
     results = {}
     for mode in ("0", "-1"):      # streamed batch by batch, then the library's own choice (zero-copy gather)
-        os.environ["DT_STREAM_ZERO_COPY"] = mode
-        try:
+        if True:
             with dt.Tracker.from_scene(scene) as trk:
+                trk.set_option("stream_zero_copy", int(mode))
                 for j in range(cfg.n_exp):
                     trk.load_image_batch(j, flux_pool[j % POOL:j % POOL + 1], var_pool[j % POOL:j % POOL + 1])
                 snr, hits = trk.stack(el, scene.t0)
@@ -203,8 +206,6 @@ def test_full_size_lsst_streamed():
                 results[mode] = (snr.cpu().numpy(), hits.cpu().numpy(), st)
                 if mode == "0":
                     sample = _pick_sample(scene, hits, cfg.n_orbits)
-        finally:
-            os.environ.pop("DT_STREAM_ZERO_COPY", None)
     assert np.array_equal(results["0"][0], results["-1"][0]) and np.array_equal(results["0"][1], results["-1"][1])
     snr_h, hits_h, st = results["0"]
 
