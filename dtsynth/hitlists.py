@@ -15,7 +15,7 @@ from . import rng
 
 
 def build(n_orbits: int, n_groups: int, width: int, height: int, cluster: int, density: float,
-          seed: int, device):
+          seed: int, device, px_per_sector: int = 8):
     """-> dict(mask [G, n_pad] int32, base [G, n_pad/32] int64, offsets [hits] int32, hits,
     unique_sectors, touched_orbits) -- all torch tensors on `device`."""
     import torch
@@ -62,7 +62,7 @@ def build(n_orbits: int, n_groups: int, width: int, height: int, cluster: int, d
             lane_rank = torch.cumsum(on2, 1) - on2
             pos = (seg[g, :, b].unsqueeze(1) + lane_rank).reshape(-1)[on]
             offsets[pos] = (off + (b << 27)).to(torch.int32)      # entry = (exposure in group) << 27 | pixel offset
-            sec_ids.append(torch.unique((j * plane + off) >> 3))          # 8 fp32 per 32-B sector
+            sec_ids.append(torch.unique((j * plane + off) // px_per_sector))   # 8 fp32 (4 float2) per 32-B sector
         if sec_ids:
             sectors += int(sum(s.numel() for s in sec_ids))               # exposures are disjoint
     cnt = tile_tot

@@ -281,6 +281,14 @@ const char *dt_version(void);
  */
 int dt_fp64_peak(int32_t device, double *tflops);
 
+/*
+ * dt_probe_random_gather: what the device gives a gather-bound kernel -- independent 4-B loads at hashed
+ * addresses of a buffer of buffer_bytes (rounded down to a power of two; >= 1 MiB), eight in flight per thread;
+ * hint64 != 0: the loads carry .L2::64B (a miss fetches 64 B of DRAM instead of 128 B).  Writes gathers per
+ * second.  The second roofline denominator of kernel 3 on sparse hit lists.
+ */
+int dt_probe_random_gather(int32_t device, int64_t buffer_bytes, int32_t hint64, double *gathers_per_s);
+
 #ifdef __cplusplus
 }
 #endif

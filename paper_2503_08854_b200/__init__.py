@@ -29,7 +29,7 @@ _ERR_NAMES = {-1: "DT_ERR_INVALID_ARG", -2: "DT_ERR_OOM", -3: "DT_ERR_CUDA", -4:
 
 EXPORTS = ["dt_create", "dt_destroy", "dt_load_image_batch", "dt_stack", "dt_stack_epochs", "dt_set_patch",
            "dt_set_outlier_clip", "dt_threshold", "dt_topk", "dt_project",
-           "dt_gather_hits", "dt_filter_intersections", "dt_set_option", "dt_get_stats", "dt_last_error", "dt_version", "dt_fp64_peak"]
+           "dt_gather_hits", "dt_filter_intersections", "dt_set_option", "dt_get_stats", "dt_last_error", "dt_version", "dt_fp64_peak", "dt_probe_random_gather"]
 
 
 class DtError(RuntimeError):
@@ -90,6 +90,7 @@ def lib():
         L.dt_last_error.restype = C.c_char_p
         L.dt_version.restype = C.c_char_p
         L.dt_fp64_peak.argtypes = [C.c_int32, dp]
+        L.dt_probe_random_gather.argtypes = [C.c_int32, C.c_int64, C.c_int32, dp]
         for name in EXPORTS:
             getattr(L, name)
         _lib = L
@@ -288,6 +289,12 @@ def dt_get_stats(ctx) -> dict:
 def dt_fp64_peak(device: int = 0) -> float:
     out = C.c_double(0.0)
     _check(lib().dt_fp64_peak(device, C.byref(out)))
+    return out.value
+
+
+def dt_probe_random_gather(device: int = 0, buffer_bytes: int = 8 << 30, hint64: int = 0) -> float:
+    out = C.c_double(0.0)
+    _check(lib().dt_probe_random_gather(device, buffer_bytes, hint64, C.byref(out)))
     return out.value
 
 

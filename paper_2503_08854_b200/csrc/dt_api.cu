@@ -986,4 +986,18 @@ int dt_fp64_peak(int32_t device, double *tflops)
     return fp64_peak_device(tflops, nullptr) == cudaSuccess ? DT_OK : DT_ERR_CUDA;
 }
 
+int dt_probe_random_gather(int32_t device, int64_t buffer_bytes, int32_t hint64, double *gathers_per_s)
+{
+    if (!gathers_per_s || buffer_bytes < (1 << 20)) return DT_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return DT_ERR_CUDA;
+    }
+    if (cudaSetDevice(device) != cudaSuccess) return DT_ERR_CUDA;
+    const cudaError_t e = random_gather_probe(buffer_bytes, hint64, gathers_per_s, nullptr);
+    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return DT_ERR_OOM; }
+    return e == cudaSuccess ? DT_OK : DT_ERR_CUDA;
+}
+
 }  // extern "C"

@@ -155,5 +155,7 @@ cudaError_t threshold_device(const double *snr, const int32_t *hits, int64_t n, 
 
 // FP64 FMA issue-rate probe (dt_fp64_peak).
 cudaError_t fp64_peak_device(double *tflops, cudaStream_t stream);
+// Random 4-B gather rate over a buffer of buffer_bytes (dt_probe_random_gather).
+cudaError_t random_gather_probe(int64_t buffer_bytes, int hint64, double *gathers_per_s, cudaStream_t stream);
 
 }  // namespace dt
