@@ -707,6 +707,18 @@ def main():
     clocks = entry.pop("clocks", None)
     main_cfg = w.cfg
     n_main = w.n
+    topk_ms = {}
+    if rank == 0:                                      # device top-k / threshold over the step's per-orbit SNR
+        for k in (64, 4096):
+            w.trk.topk(k, min_hits=1)
+            t0 = time.perf_counter()
+            for _ in range(5):
+                w.trk.topk(k, min_hits=1)
+            topk_ms["k=%d" % k] = (time.perf_counter() - t0) / 5 * 1e3
+        t0 = time.perf_counter()
+        _i, _v, nf = w.trk.threshold(5.0, min_hits=1)
+        topk_ms["threshold snr>=5"] = (time.perf_counter() - t0) * 1e3
+        topk_ms["n_above_5"] = int(nf)
     controlled = []
     if rank == 0 and main_cfg.name == "small_mba" and not args.no_gather_bench:
         controlled = gather_bench(dt, w.trk, w.cfg, dev, hbm_gbs, flush, args.gather_reps, pick_regimes(args))
@@ -733,7 +745,7 @@ def main():
                 "roofline": k1, "step_roofline": entry.get("roofline"),
                 "stages_ms": entry["stages_ms"], "hits_per_step": entry["hits_per_step"],
                 "cold_solves": entry["cold_solves"], "substep_solves": entry["substep_solves"],
-                "peaks": peaks, "wall_s_timed_region": wall}
+                "topk_ms": topk_ms, "peaks": peaks, "wall_s_timed_region": wall}
 
     # ---- every BASELINE.json config, literal and focused, at full size ----
     configs, gather_regimes, skipped = [entry], list(controlled), []

@@ -115,6 +115,9 @@ typedef struct {
     int32_t propagate_launches, gather_launches;
     int32_t image_zero_copy;   /* 1 when a streamed survey was gathered straight from the pinned host     */
                                /* planes (few hits) instead of being copied batch by batch               */
+    int32_t image_tiles;       /* 1 when a streamed survey went through the tiled image cache: only the   */
+                               /* 64 x 64-pixel tiles the hits fall on were copied (h2d_image_bytes)       */
+    int64_t tiles_fetched;     /* tiles copied host -> device by the call                                 */
 } dt_stats;
 
 /*
@@ -134,11 +137,14 @@ int dt_destroy(dt_context *ctx);
  *     are COPIED into the context's image store in HBM and the caller may free them on return;
  *   - otherwise (streaming mode; north_star subsystem 4) the library RETAINS the pointers: they
  *     must be DT_MEM_PINNED (else DT_ERR_INVALID_ARG) and stay valid until dt_destroy or until the
- *     same exposure range is loaded again; dt_stack then streams them in double-buffered batches --
- *     or, when a probe of the hit density predicts that the gathers would move less than 5 % of the
- *     bytes streaming would (a blind search), copies no image and gathers the hit pixels straight
- *     from the (device-mapped) page-locked planes; results are bit-identical either way
- *     (dt_stats.image_zero_copy says which way was taken).
+ *     same exposure range is loaded again.  dt_stack then runs the search first (it needs no image) and
+ *     moves only what the hits need: when a probe of the hit density predicts
+ *     that the gathers would move less than 5 % of the bytes the planes hold (a blind search) no image is
+ *     copied and the hit pixels are read straight from the (device-mapped) page-locked planes; otherwise
+ *     the 64 x 64-pixel TILES the hits fall on are copied into a device tile cache (tiles with few hits stay
+ *     zero-copy).  Planes that are not device-mappable (or "stream_tiles" = 0) are streamed whole, in
+ *     double-buffered batches.  Results are bit-identical in every case (dt_stats.image_zero_copy,
+ *     image_tiles, tiles_fetched, h2d_image_bytes say what was done).
  * Ranges may be loaded in any order and re-loaded; overlapping a previously loaded range replaces it.
  */
 int dt_load_image_batch(dt_context *ctx, int32_t first_exposure, int32_t count, const float *flux,
@@ -261,6 +267,9 @@ int dt_filter_intersections(dt_context *ctx, const double *elements, int64_t n, 
  *   "gather_window"       dense schedule: exposures the fastest CTA may be ahead (0 = from the L2 size)
  *   "gather_prefetch"     dense schedule: planes ahead of the L2 prefetch sweep (0 = off)
  *   "gather_l1"           dense schedule: 1 pixel loads allocate in L1, 0 they do not
+ *   "stream_tiles"        streaming mode: -1 / 1 use the tiled image cache when the planes are device-mappable
+ *                         (default), 0 stream whole planes in double-buffered batches; "tile_min_hits": hits of
+ *                         one orbit unit on a tile from which the tile is fetched (0 = tile bytes / 256)
  *   "stream_zero_copy"    streaming mode: -1 probe the hit density (default), 0 always copy batches, 1 always
  *                         gather from the pinned planes
  *   "zero_copy_elements"  1 kernel 1 reads DT_MEM_PINNED elements in place (default), 0 copies them first

@@ -55,7 +55,8 @@ class dt_stats(C.Structure):
                 ("substep_solves", C.c_int64), ("h2d_image_bytes", C.c_int64), ("streamed", C.c_int32), ("n_image_batches", C.c_int32),
                 ("ms_total", C.c_float), ("ms_propagate", C.c_float), ("ms_gather", C.c_float),
                 ("ms_finalize", C.c_float), ("launches", C.c_int32), ("propagate_launches", C.c_int32),
-                ("gather_launches", C.c_int32), ("image_zero_copy", C.c_int32)]
+                ("gather_launches", C.c_int32), ("image_zero_copy", C.c_int32), ("image_tiles", C.c_int32),
+                ("tiles_fetched", C.c_int64)]
 
 
 _lib = None

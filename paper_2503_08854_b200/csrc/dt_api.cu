@@ -25,6 +25,7 @@ namespace {
 constexpr int64_t kMaxUnitOrbits = 1 << 20;   // orbits per work unit (bounds the hit buffer)
 constexpr int32_t kMaxUnitExposures = 512;    // exposures per work unit (16 groups)
 constexpr int kMinCtas = 148 * 4;             // fill the machine before giving up exposure splits
+constexpr int kTileLog2 = 6;                  // streaming tile cache: 64 x 64-pixel tiles (16 KB of fp32 per plane)
 
 struct Timer {
     cudaEvent_t a = nullptr, b = nullptr;
@@ -81,6 +82,15 @@ struct dt_context {
     int32_t sm_count = 0;                               // SMs of this context's device
     int32_t stream_zero_copy = -1;                      // -1 decide from a probe, 0 never, 1 always
     const float **d_flux_ptrs = nullptr, **d_var_ptrs = nullptr;   // [N] device-mapped pinned planes (zero-copy gather)
+    // streaming mode, tiled image cache (dt_tiles.cu)
+    int32_t stream_tiles = -1;                          // -1 / 1: use it when the planes are device-mappable, 0: never
+    int32_t tile_min_hits = 0;                          // 0: default (a tile's bytes / 256)
+    int32_t *tile_count = nullptr, *tile_slot = nullptr;
+    unsigned int *tile_alloc = nullptr;
+    uint2 *tile_fetch = nullptr;
+    float *tile_buf = nullptr;
+    int32_t tile_capacity = 0, tiles_x = 0, tiles_per_plane = 0;
+    int64_t slot_floats = 0;
     bool zero_copy_elements = true;                     // false: copy pinned elements to the device first
     std::vector<cudaEvent_t> ev_pool;                   // timing events
 
@@ -151,6 +161,11 @@ void free_all(dt_context *c)
     cudaFree(c->d_offsets);
     cudaFree(c->d_counters);
     cudaFree(c->d_progress);
+    cudaFree(c->tile_count);
+    cudaFree(c->tile_slot);
+    cudaFree(c->tile_alloc);
+    cudaFree(c->tile_fetch);
+    cudaFree(c->tile_buf);
     cudaFree((void *)c->d_flux_ptrs);
     cudaFree((void *)c->d_var_ptrs);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
@@ -199,10 +214,16 @@ int32_t pick_gather_window(const dt_context *c)
 
 int mem_kind_ok(int32_t k) { return k == DT_MEM_HOST || k == DT_MEM_PINNED || k == DT_MEM_DEVICE; }
 
-int ensure_store(dt_context *c)
+// Streaming mode, whole-plane double buffering: two device slots of batch_exp exposures each.
+int ensure_stream_slots(dt_context *c)
 {
-    if (c->streaming) {
+    {
         if (c->d_buf_flux[0]) return DT_OK;
+        if (c->tile_buf) {                    // the tile cache and the plane slots share the image budget
+            cudaFree(c->tile_buf);
+            c->tile_buf = nullptr;
+            c->tile_capacity = 0;
+        }
         const int64_t per_exp = c->plane * 4 * (c->var_mode == 1 ? 2 : 1);
         int64_t b = c->budget / (2 * per_exp);
         if (b < 1) return fail(c, DT_ERR_OOM, "hbm_budget_bytes %lld cannot hold two exposures of %lld bytes",
@@ -219,6 +240,44 @@ int ensure_store(dt_context *c)
         }
         return DT_OK;
     }
+}
+
+// Streaming mode, tiled image cache (dt_tiles.cu): count / slot tables for one exposure unit and as many tile
+// slots as the image budget holds.
+int ensure_tile_cache(dt_context *c)
+{
+    const int32_t ts = 1 << kTileLog2;
+    c->tiles_x = (c->W + ts - 1) / ts;
+    c->tiles_per_plane = c->tiles_x * ((c->H + ts - 1) / ts);
+    c->slot_floats = (int64_t)ts * ts * (c->var_mode == 1 ? 2 : 1);
+    if (c->tile_buf) return DT_OK;
+    for (int s = 0; s < 2; ++s) {             // the plane slots and the tile cache share the image budget
+        cudaFree(c->d_buf_flux[s]);
+        cudaFree(c->d_buf_var[s]);
+        c->d_buf_flux[s] = c->d_buf_var[s] = nullptr;
+    }
+    const size_t cells = (size_t)kMaxUnitExposures * (size_t)c->tiles_per_plane;
+    if (!c->tile_count) {
+        CU(c, cudaMalloc((void **)&c->tile_count, cells * sizeof(int32_t)));
+        CU(c, cudaMemsetAsync(c->tile_count, 0, cells * sizeof(int32_t), c->stream));
+        CU(c, cudaMalloc((void **)&c->tile_slot, cells * sizeof(int32_t)));
+        CU(c, cudaMalloc((void **)&c->tile_alloc, 8 * sizeof(unsigned int)));
+        CU(c, cudaMemsetAsync(c->tile_alloc, 0, 8 * sizeof(unsigned int), c->stream));
+    }
+    int64_t cap = c->budget / (c->slot_floats * 4);
+    cap = std::min<int64_t>(cap, (int64_t)cells);            // every tile of the unit resident: nothing more to gain
+    if (cap < 1) return fail(c, DT_ERR_OOM, "hbm_budget_bytes %lld cannot hold one image tile", (long long)c->budget);
+    CU(c, cudaMalloc((void **)&c->tile_buf, (size_t)cap * (size_t)c->slot_floats * 4));
+    cudaFree(c->tile_fetch);
+    c->tile_fetch = nullptr;
+    CU(c, cudaMalloc((void **)&c->tile_fetch, (size_t)cap * sizeof(uint2)));
+    c->tile_capacity = (int32_t)std::min<int64_t>(cap, 0x7fffffff);
+    return DT_OK;
+}
+
+int ensure_store(dt_context *c)
+{
+    if (c->streaming) return DT_OK;           // streaming buffers are created by the path dt_stack takes
     if (c->var_mode == 1) {
         if (!c->d_fv) CU(c, cudaMalloc((void **)&c->d_fv, (size_t)(c->N * c->plane) * 8));
     } else if (!c->d_flux) {
@@ -457,9 +516,12 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
     if (n == 0) { c->n_last = 0; return DT_OK; }
 
     // ---- buffers ----
-    const int32_t unit_exp = c->streaming ? c->batch_exp : std::min<int32_t>(c->N, kMaxUnitExposures);
+    // an exposure unit is at most 512 exposures; only the whole-plane streaming path uses smaller ones (its
+    // double-buffered batches), decided below
+    const int32_t unit_exp_max = std::min<int32_t>(c->N, kMaxUnitExposures);
+    int32_t unit_exp = unit_exp_max;
     const int64_t unit_orb = std::min<int64_t>((n + 31) / 32 * 32, kMaxUnitOrbits);
-    const int32_t unit_groups = (unit_exp + kGroup - 1) / kGroup;
+    const int32_t unit_groups = (unit_exp_max + kGroup - 1) / kGroup;
     // Elements: kernel 1 stages each tile with one bulk copy, from device memory or straight from
     // page-locked host memory (first pass over the orbits; it leaves a device copy for later passes
     // and for the finalisation).  Pageable or misaligned inputs are copied to the device first.
@@ -505,8 +567,7 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
     CU(c, grow(c->d_mask, c->mask_cap, unit_orb * unit_groups));
     CU(c, grow(c->d_base, c->base_cap, (unit_orb / 32) * unit_groups));
     CU(c, grow(c->d_offsets, c->off_cap, unit_orb * (int64_t)unit_groups * kGroup));
-    const int n_units_total = (int)(((c->N + unit_exp - 1) / unit_exp) * ((n + unit_orb - 1) / unit_orb));
-    while ((int64_t)c->ev_pool.size() < 4 + 3 * (int64_t)n_units_total) {
+    while ((int64_t)c->ev_pool.size() < 4) {
         cudaEvent_t e;
         CU(c, cudaEventCreate(&e));
         c->ev_pool.push_back(e);
@@ -521,8 +582,6 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
     CU(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
 
     const int mode = propagate_mode(c);
-    const int n_batches = (c->N + unit_exp - 1) / unit_exp;
-    st.n_image_batches = n_batches;
 
     auto issue_copy = [&](int b) -> int {
         const int slot = b & 1;
@@ -550,9 +609,10 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
     // would move less than 5 % of the bytes streaming would, no image is copied at all and the sparse
     // gather reads the hit pixels over PCIe.  Same pixels, same arithmetic: bit-identical results.
     bool zero_copy_images = false;
-    if (c->streaming && c->stream_zero_copy != 0) {
+    bool mappable = false;
+    if (c->streaming && (c->stream_zero_copy != 0 || c->stream_tiles != 0)) {
         std::vector<const float *> hf(c->N), hv(c->N, nullptr);
-        bool mappable = true;
+        mappable = true;
         for (int32_t j = 0; j < c->N && mappable; ++j) {
             void *d = nullptr;
             mappable = cudaHostGetDevicePointer(&d, const_cast<float *>(c->h_flux[j]), 0) == cudaSuccess && d;
@@ -573,9 +633,9 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
                                   cudaMemcpyHostToDevice, c->stream));
             if (c->stream_zero_copy == 1) {
                 zero_copy_images = true;
-            } else {
+            } else if (c->stream_zero_copy != 0) {
                 const int64_t no = std::min<int64_t>(unit_orb, n);
-                const int32_t ne = std::min<int32_t>(unit_exp, c->N);
+                const int32_t ne = std::min<int32_t>(unit_exp_max, c->N);
                 PropagateParams p;
                 fill_common(c, p, t0);
                 p.elements = first_src;
@@ -603,7 +663,35 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
     }
     st.image_zero_copy = zero_copy_images ? 1 : 0;
 
+    // ---- streaming mode, many hits: hits first, then only the image TILES the hits fall on cross PCIe, into a
+    // device tile cache (dt_tiles.cu; PAPER.md:192 tiled layout, PAPER.md:330-332 pipelining); whole-plane double
+    // buffering remains for planes that are not device-mappable or when the cache is switched off ----
+    bool tiled = false;
     if (c->streaming && !zero_copy_images) {
+        if (mappable && c->stream_tiles != 0) {
+            rc = ensure_tile_cache(c);
+            if (rc != DT_OK) return rc;
+            tiled = true;
+            CU(c, cudaMemsetAsync(c->tile_alloc, 0, 8 * sizeof(unsigned int), c->stream));
+        } else {
+            rc = ensure_stream_slots(c);
+            if (rc != DT_OK) return rc;
+            unit_exp = c->batch_exp;
+        }
+    }
+    st.image_tiles = tiled ? 1 : 0;
+    const int n_batches = (c->N + unit_exp - 1) / unit_exp;
+    st.n_image_batches = n_batches;
+    {
+        const int64_t n_units_total = (int64_t)n_batches * ((n + unit_orb - 1) / unit_orb);
+        while ((int64_t)c->ev_pool.size() < 4 + 3 * n_units_total) {
+            cudaEvent_t e;
+            CU(c, cudaEventCreate(&e));
+            c->ev_pool.push_back(e);
+        }
+    }
+
+    if (c->streaming && !zero_copy_images && !tiled) {
         // the copy stream must not start before earlier work on the context stream that may still
         // read the slots (a previous dt_stack) has been ordered: previous calls synchronise, so
         // only the free events of this call matter
@@ -615,9 +703,13 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
     for (int b = 0; b < n_batches; ++b) {
         const int slot = b & 1;
         const int32_t first = b * unit_exp, n_exp = std::min<int32_t>(unit_exp, c->N - first);
-        if (c->streaming && !zero_copy_images && b + 1 < n_batches) {
+        if (c->streaming && !zero_copy_images && !tiled && b + 1 < n_batches) {
             rc = issue_copy(b + 1);
             if (rc != DT_OK) return rc;
+        }
+        if (tiled) {       // a fresh cache for this exposure unit: no tile resident, no slot handed out
+            CU(c, cudaMemsetAsync(c->tile_slot, 0xff, (size_t)n_exp * (size_t)c->tiles_per_plane * sizeof(int32_t), c->stream));
+            CU(c, cudaMemsetAsync(c->tile_alloc, 0, sizeof(unsigned int), c->stream));
         }
         bool waited = false;
         for (int64_t o0 = 0; o0 < n; o0 += unit_orb) {
@@ -643,12 +735,46 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
             st.propagate_launches += 1;
             CU(c, cudaEventRecord(ev_at(3 * unit_idx + 1), c->stream));
 
-            if (c->streaming && !zero_copy_images && !waited) {
+            if (c->streaming && !zero_copy_images && !tiled && !waited) {
                 CU(c, cudaStreamWaitEvent(c->stream, c->ev_ready[slot], 0));
                 waited = true;
             }
             GatherParams g;
             memset(&g, 0, sizeof g);
+            if (tiled) {
+                TileParams t;
+                memset(&t, 0, sizeof t);
+                t.n_pad = p.n_pad;
+                t.n_groups = (n_exp + kGroup - 1) / kGroup;
+                t.mask = c->d_mask;
+                t.base = c->d_base;
+                t.offsets = c->d_offsets;
+                t.n_exp = n_exp;
+                t.first_exposure = first;
+                t.width = c->W;
+                t.height = c->H;
+                t.ts_log2 = kTileLog2;
+                t.tiles_x = c->tiles_x;
+                t.tiles_per_plane = c->tiles_per_plane;
+                t.tile_count = c->tile_count;
+                t.tile_slot = c->tile_slot;
+                t.alloc = c->tile_alloc;
+                t.capacity = c->tile_capacity;
+                t.min_hits = c->tile_min_hits > 0 ? c->tile_min_hits : (int32_t)std::max<int64_t>(1, c->slot_floats * 4 / 256);
+                t.fetch_list = c->tile_fetch;
+                t.flux_ptrs = c->d_flux_ptrs;
+                t.var_ptrs = (c->var_mode == 1) ? c->d_var_ptrs : nullptr;
+                t.tile_buf = c->tile_buf;
+                t.slot_floats = c->slot_floats;
+                CU(c, launch_tiles(t, c->sm_count, c->stream));
+                g.tile_slot = c->tile_slot;
+                g.tile_buf = c->tile_buf;
+                g.slot_floats = c->slot_floats;
+                g.ts_log2 = kTileLog2;
+                g.tiles_x = c->tiles_x;
+                g.tiles_per_plane = c->tiles_per_plane;
+                g.tile_e0 = first;
+            }
             g.n_orbits = no;
             g.n_pad = p.n_pad;
             g.first_exposure = first;
@@ -656,7 +782,7 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
             g.mask = c->d_mask;
             g.base = c->d_base;
             g.offsets = c->d_offsets;
-            if (zero_copy_images) {
+            if (zero_copy_images || tiled) {
                 g.flux_ptrs = c->d_flux_ptrs;
                 g.var_ptrs = (c->var_mode == 1) ? c->d_var_ptrs : nullptr;
             } else if (c->streaming) {
@@ -674,7 +800,7 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
             g.progress = c->d_progress;
             g.window = c->gather_window;
             g.n_hits_dev = c->d_counters;            // the unit's hit allocator, final after kernel 1
-            g.lockstep_mode = zero_copy_images ? 0 : c->gather_lockstep;
+            g.lockstep_mode = (zero_copy_images || tiled) ? 0 : c->gather_lockstep;
             g.ld_cached = c->gather_ld_cached;
             g.prefetch = c->streaming ? 0 : c->gather_prefetch;
             g.n_exp_store = c->N;
@@ -685,7 +811,7 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
             CU(c, cudaEventRecord(ev_at(3 * unit_idx + 2), c->stream));
             unit_idx += 1;
         }
-        if (c->streaming && !zero_copy_images) {
+        if (c->streaming && !zero_copy_images && !tiled) {
             CU(c, cudaEventRecord(c->ev_free[slot], c->stream));
             c->ev_free_recorded[slot] = true;
         }
@@ -700,8 +826,12 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
         CU(c, cudaMemcpyAsync(hits_out, c->d_hits, (size_t)n * 4, cudaMemcpyDefault, c->stream));
     CU(c, cudaEventRecord(c->ev_pool[1], c->stream));
     unsigned long long hc[8];
+    unsigned int tc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     CU(c, cudaMemcpyAsync(hc, c->d_counters, sizeof hc, cudaMemcpyDeviceToHost, c->stream));
+    if (tiled) CU(c, cudaMemcpyAsync(tc, c->tile_alloc, sizeof tc, cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
+    st.tiles_fetched = (int64_t)tc[2];
+    st.h2d_image_bytes += (int64_t)tc[2] * c->slot_floats * 4;
     CU(c, cudaEventElapsedTime(&st.ms_total, c->ev_pool[0], c->ev_pool[1]));
     CU(c, cudaEventElapsedTime(&st.ms_finalize, c->ev_pool[2], c->ev_pool[3]));
     for (int u = 0; u < unit_idx; ++u) {
@@ -957,6 +1087,10 @@ int dt_set_option(dt_context *c, const char *name, int64_t value)
         c->gather_prefetch = (int32_t)std::max<int64_t>(0, std::min<int64_t>(value, 8));
     } else if (k == "gather_l1") {
         c->gather_ld_cached = value ? 1 : 0;
+    } else if (k == "stream_tiles") {
+        c->stream_tiles = value < 0 ? -1 : (value ? 1 : 0);
+    } else if (k == "tile_min_hits") {
+        c->tile_min_hits = (int32_t)std::max<int64_t>(0, std::min<int64_t>(value, 1 << 30));
     } else if (k == "stream_zero_copy") {
         c->stream_zero_copy = value < 0 ? -1 : (value ? 1 : 0);
     } else if (k == "zero_copy_elements") {

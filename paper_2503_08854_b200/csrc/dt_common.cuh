@@ -99,8 +99,38 @@ struct GatherParams {
     int32_t patch;              // k >= 1, odd
     const double *patch_w;      // device [k*k] row-major, or NULL (all 1)
     double clip;                // +inf: no rejection
-    int32_t width, height;      // image size (patch bounds)
+    int32_t width, height;      // image size (patch bounds, tile lookup)
+    // tiled image cache (dt_tiles.cu; streaming mode): slot of tile (exposure - tile_e0, tile) or -1; a pixel
+    // without a slot is read from flux_ptrs / var_ptrs (zero-copy).  NULL: no cache.
+    const int32_t *tile_slot;   // [<= 512 exposures][tiles_per_plane]
+    const float *tile_buf;      // slot s at tile_buf + s * slot_floats: ts*ts flux values, then ts*ts variances (plane mode)
+    int64_t slot_floats;
+    int32_t ts_log2, tiles_x, tiles_per_plane;
+    int32_t tile_e0;            // absolute exposure of row 0 of tile_slot
 };
+
+// ---- tiled image cache of the streaming mode (dt_tiles.cu) -------------------------------------------------------
+struct TileParams {
+    int64_t n_pad;              // hit list of the unit (format: dtrack.h dt_gather_hits)
+    int32_t n_groups;
+    const uint32_t *mask;
+    const unsigned long long *base;
+    const uint32_t *offsets;
+    int32_t n_exp;              // exposures of the unit (rows of tile_count / tile_slot in use)
+    int32_t first_exposure;     // absolute index of the unit's first exposure (row 0)
+    int32_t width, height, ts_log2, tiles_x, tiles_per_plane;
+    int32_t *tile_count;        // [n_exp][tiles_per_plane], zero on entry and on exit
+    int32_t *tile_slot;         // [n_exp][tiles_per_plane], -1 = not resident
+    unsigned int *alloc;        // [0] slots handed out in this exposure unit, [1] fetch queue length, [2] tiles fetched (statistics)
+    int32_t capacity;           // slots of tile_buf
+    int32_t min_hits;           // a tile is fetched once a unit has at least this many hits on it
+    uint2 *fetch_list;          // [capacity]: (row * tiles_per_plane + tile, slot)
+    const float *const *flux_ptrs;   // device-mapped page-locked host planes, absolute exposure index
+    const float *const *var_ptrs;    // NULL in scalar-variance mode
+    float *tile_buf;
+    int64_t slot_floats;
+};
+cudaError_t launch_tiles(const TileParams &t, int sm_count, cudaStream_t stream);
 
 // A hit entry is (exposure within its group) << kOffsetBits | (iy * W + ix): an entry names its exposure, so
 // a block of the list can be processed as one flat coalesced list.  W * H <= 2^27 (dt_create checks).

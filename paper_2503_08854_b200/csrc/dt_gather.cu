@@ -32,6 +32,22 @@ namespace dt {
 
 constexpr int kSparseThreads = 256;
 
+// Tiled image cache (dt_tiles.cu): the pixel (exposure j, offset a) from its tile's slot when the tile is resident.
+template <bool PLANE_VAR>
+__device__ __forceinline__ bool load_pixel_tiled(const GatherParams &p, int64_t j, uint32_t a, float &f, float &v)
+{
+    const uint32_t y = a / (uint32_t)p.width, x = a - y * (uint32_t)p.width;
+    const int tile = (int)(y >> p.ts_log2) * p.tiles_x + (int)(x >> p.ts_log2);
+    const int32_t s = p.tile_slot[(j - p.tile_e0) * p.tiles_per_plane + tile];
+    if (s < 0) return false;
+    const uint32_t m = (1u << p.ts_log2) - 1u;
+    const uint32_t k = ((y & m) << p.ts_log2) + (x & m);
+    const float *t = p.tile_buf + (int64_t)s * p.slot_floats;
+    f = ld_pixel_cached(t + k);
+    if (PLANE_VAR) v = ld_pixel_cached(t + (1u << (2 * p.ts_log2)) + k);
+    return true;
+}
+
 // One pixel of the extended stack (any store: resident planes, interleaved (flux, var), or device-mapped
 // host planes): fp32 values widened to fp64; v is the exposure's scalar in scalar-variance mode.
 template <bool PLANE_VAR>
@@ -39,6 +55,12 @@ __device__ __forceinline__ void load_pixel_any(const GatherParams &p, int64_t j,
                                                double &v)
 {
     if (p.flux_ptrs) {
+        float ff, vv = 0.f;
+        if (p.tile_slot && load_pixel_tiled<PLANE_VAR>(p, j, (uint32_t)a, ff, vv)) {
+            f = (double)ff;
+            v = PLANE_VAR ? (double)vv : v_scalar;
+            return;
+        }
         f = (double)ld_pixel_cached(p.flux_ptrs[j] + a);
         v = PLANE_VAR ? (double)ld_pixel_cached(p.var_ptrs[j] + a) : v_scalar;
     } else if (PLANE_VAR && p.fv) {
@@ -159,9 +181,12 @@ __global__ void __launch_bounds__(kSparseThreads) k_gather_sparse(const GatherPa
                 vv[q] = 1.f;
                 if (have[q]) {
                     if (p.flux_ptrs) {
-                        // zero-copy: the pixel comes straight from page-locked host memory over PCIe
-                        f[q] = ld_pixel_cached(p.flux_ptrs[j0 + jj[q]] + off[q]);
-                        if (PLANE_VAR) vv[q] = ld_pixel_cached(p.var_ptrs[j0 + jj[q]] + off[q]);
+                        // streaming mode: from the tile cache when the pixel's tile is resident, else
+                        // zero-copy: straight from page-locked host memory over PCIe
+                        if (!(p.tile_slot && load_pixel_tiled<PLANE_VAR>(p, j0 + jj[q], off[q], f[q], vv[q]))) {
+                            f[q] = ld_pixel_cached(p.flux_ptrs[j0 + jj[q]] + off[q]);
+                            if (PLANE_VAR) vv[q] = ld_pixel_cached(p.var_ptrs[j0 + jj[q]] + off[q]);
+                        }
                     } else if (PLANE_VAR && p.fv) {
                         const float2 t2 = ld_pixel2_64(p.fv + ((j0 + jj[q]) * p.plane + off[q]));
                         f[q] = t2.x;

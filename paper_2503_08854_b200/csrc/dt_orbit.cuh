@@ -341,14 +341,29 @@ __device__ __forceinline__ Kepler kepler_warm_finish(double e, const Kepler &K0,
 
 // LOW = 3 for the exposure-to-exposure step, 2 for the light-time re-solve: the warp takes the cheaper
 // order when every lane's step is inside its domain (one vote), else ORDER 4.  All 32 lanes must call.
+// One Newton step on a seed-quality reciprocal (1e-6 -> 1e-12) and the quantities derived from it: an ORDER 4
+// series (steps up to 0.04 rad) steered by the bare seed would leave 7e-15 rad after the polish at e = 0.9.
+__device__ __forceinline__ void warm_refine_rg(WarmPre &w)
+{
+    const double g = 1.0 - w.ec;
+    const double f0 = -w.x * g;                          // x = -f0 rg with the seed rg ~ 1/g
+    w.rg = w.rg * fma(-g, w.rg, 2.0);
+    w.x = -f0 * w.rg;
+    w.a2 = 0.5 * w.es * w.rg;
+}
+
+// The series of a POLISHED step is steered by the MUFU seed of 1/g alone (1e-6 relative: theta is off by
+// <= 1e-6 |x| <= 1.5e-8 rad in the ORDER <= 3 domains, of which the Newton polish -- with its own refined
+// reciprocal -- leaves a2 (1.5e-8)^2 < 1e-15); the ORDER 4 domain refines the reciprocal first.
 template <int LOW>
 __device__ __forceinline__ Kepler kepler_warm(double e, const Kepler &K0, double Mn, bool &ok)
 {
-    const WarmPre w = kepler_warm_pre(e, K0, Mn);
+    WarmPre w = kepler_warm_pre(e, K0, Mn, true);
     if (__all_sync(0xffffffffu, kepler_warm_in_domain<LOW>(w))) {
         ok = true;
         return kepler_warm_finish<LOW>(e, K0, Mn, w);
     }
+    warm_refine_rg(w);
     ok = kepler_warm_in_domain<4>(w);
     return kepler_warm_finish<4>(e, K0, Mn, w);
 }

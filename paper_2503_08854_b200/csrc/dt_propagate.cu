@@ -137,7 +137,9 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 bool solved = false;
                 unpolished = false;
                 if (have_state) {
-                    const WarmPre w = kepler_warm_pre(o.e, K, M, PRECULL && !prev_refined);
+                    // the series is steered by the MUFU seed of 1/g in every mode (dt_orbit.cuh kepler_warm);
+                    // the polished ORDER 4 step refines it first
+                    WarmPre w = kepler_warm_pre(o.e, K, M, true);
                     if (__all_sync(0xffffffffu, kepler_warm_in_domain<3>(w))) {
                         // with the pre-cull the precision is deferred to the pairs that survive it
                         // (a warp whose last pair survived the cull -- a focused search -- polishes at
@@ -160,6 +162,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                             unpolished = true;
                             since_sync += 1;
                         } else {
+                            warm_refine_rg(w);
                             K = kepler_warm_finish<4>(o.e, K, M, w);
                         }
                         solved = true;
@@ -247,7 +250,8 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                     const double az0 = fma(o.Az, X0p, fma(o.Bz, K.s, -x.Rz));
                     rho2r = fma(ax0, ax0, fma(ay0, ay0, az0 * az0));
                 }
-                const double rho0 = WARM ? sqrt_nr<2>(rho2r) : sqrt(rho2r);
+                // one Goldschmidt step from the MUFU seed: 1.5e-12 relative, i.e. 3e-13 d of light-time
+                const double rho0 = WARM ? sqrt_nr<1>(rho2r) : sqrt(rho2r);
                 const double tau = rho0 * p.inv_c;
                 const double M1 = fma(o.n, dt - tau, o.M0);
                 Kepler K1;
@@ -265,7 +269,9 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 qz = fma(o.Az, X1, fma(o.Bz, K1.s, -x.Rz));
                 // ---- step 6: gnomonic projection (vector form) + pixelise ----
                 const double D = fma(qx, x.tx, fma(qy, x.ty, qz * x.tz));
-                const double inv = WARM ? rcp_nr<2>(D) : 1.0 / D;
+                // one Newton step from the MUFU seed: 1e-12 relative = 2e-9 px at the edge of a 4096-px footprint,
+                // far inside the 1e-6 px guard band
+                const double inv = WARM ? rcp_nr<1>(D) : 1.0 / D;
                 const double xe = fma(qx, x.ex, fma(qy, x.ey, qz * x.ez));
                 const double xn = fma(qx, x.nx, fma(qy, x.ny, qz * x.nz));
                 xpix = fma(xe, inv, p.cx);
@@ -273,9 +279,9 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 const double xh = xpix + 0.5, yh = ypix + 0.5;
                 // ---- step 7: footprint cull, in floating point before any integer conversion ----
                 hit = o.valid && (D > 0.0) && (xh >= 0.0) && (xh < p.W) && (yh >= 0.0) && (yh < p.H);
-                if (hit) {
-                    ix = (int32_t)floor(xh);
-                    iy = (int32_t)floor(yh);
+                if (hit) {                               // 0 <= xh < W: truncation is the floor
+                    ix = __double2int_rz(xh);
+                    iy = __double2int_rz(yh);
                 }
             }
             if (DENSE) {

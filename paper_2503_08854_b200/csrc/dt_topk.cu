@@ -67,47 +67,58 @@ __global__ void k_hist(const unsigned long long *__restrict__ keys, int64_t n, i
     if (v) atomicAdd(&hist[threadIdx.x], v);
 }
 
+// One block of 256 threads, thread d owns bin d: an inclusive suffix scan of the histogram finds the bin of the
+// k-th best key (the largest d with sum_{d' >= d} hist[d'] >= k_remaining) without walking the bins serially.
 __global__ void k_pick(int pass, int32_t k, unsigned long long *state, unsigned int *hist)
 {
-    // one thread: 256 bins, negligible
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    __shared__ unsigned long long suf[256];
+    const int t = threadIdx.x;
+    const unsigned long long c = hist[t];
+    const unsigned long long st0 = state[0], st1 = state[1], st5 = state[5], st6 = state[6];
+    suf[t] = c;
+    __syncthreads();
+    for (int off = 1; off < 256; off <<= 1) {
+        const unsigned long long v = (t + off < 256) ? suf[t + off] : 0ull;
+        __syncthreads();
+        suf[t] += v;
+        __syncthreads();
+    }
+    const unsigned long long total = suf[0];
+    const unsigned long long above = suf[t] - c;          // keys in the bins above mine
+    hist[t] = 0;                                            // every path leaves a clean histogram
     const int shift = 56 - 8 * pass;
-    unsigned long long krem = (pass == 0) ? (unsigned long long)k : state[1];
+    const unsigned long long krem = (pass == 0) ? (unsigned long long)k : st1;
     if (pass == 0) {
-        unsigned long long total = 0;
-        for (int d = 0; d < 256; ++d) total += hist[d];
-        state[2] = total;
-        state[5] = 0;
-        if (total <= krem) {   // fewer valid entries than k: take all of them
-            state[0] = 0;
-            state[1] = 0;
-            state[3] = 0;      // T = 0: every valid key is > T
-            state[4] = 0;
-            state[6] = 1;      // done flag
-            for (int d = 0; d < 256; ++d) hist[d] = 0;
+        if (total <= krem) {                                // fewer valid entries than k: take all of them
+            if (t == 0) {
+                state[0] = 0;
+                state[1] = 0;
+                state[2] = total;
+                state[3] = 0;                               // T = 0: every valid key is > T
+                state[4] = 0;
+                state[5] = 0;
+                state[6] = 1;                               // done flag
+            }
             return;
         }
-        state[6] = 0;
-    }
-    if (state[6]) {
-        for (int d = 0; d < 256; ++d) hist[d] = 0;
+        if (t == 0) {
+            state[2] = total;
+            state[6] = 0;
+        }
+    } else if (st6) {
         return;
     }
-    unsigned long long above = 0;
-    int d = 255;
-    for (; d > 0; --d) {
-        const unsigned long long c = hist[d];
-        if (above + c >= krem) break;
-        above += c;
+    // exactly one bin qualifies (k_remaining >= 1 and the bins of the current prefix hold >= k_remaining keys)
+    if (above < krem && above + c >= krem) {
+        const unsigned long long prefix = st0 | (((unsigned long long)t) << shift);
+        state[0] = prefix;
+        state[1] = krem - above;
+        state[5] = ((pass == 0) ? 0ull : st5) + above;
+        if (pass == 7) {
+            state[3] = prefix;
+            state[4] = krem - above;
+        }
     }
-    state[0] |= ((unsigned long long)d) << shift;
-    state[1] = krem - above;
-    state[5] += above;
-    if (pass == 7) {
-        state[3] = state[0];
-        state[4] = state[1];
-    }
-    for (int q = 0; q < 256; ++q) hist[q] = 0;
 }
 
 __global__ void k_count(const unsigned long long *__restrict__ keys, int64_t n,
@@ -351,7 +362,7 @@ cudaError_t topk_device(const double *snr, const int32_t *hits, int64_t n, int32
     k_keys<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(snr, hits, n, min_hits, ws.keys);
     for (int pass = 0; pass < 8; ++pass) {
         k_hist<<<nblocks, kThreads, 0, stream>>>(ws.keys, n, pass, ws.state, ws.hist);
-        k_pick<<<1, 32, 0, stream>>>(pass, (int32_t)kk64, ws.state, ws.hist);
+        k_pick<<<1, 256, 0, stream>>>(pass, (int32_t)kk64, ws.state, ws.hist);
     }
     k_count<<<nblocks, kThreads, 0, stream>>>(ws.keys, n, ws.state, ws.block_counts);
     k_scan<<<1, 1024, 0, stream>>>(ws.block_counts, nblocks, ws.state);

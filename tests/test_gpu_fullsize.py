@@ -193,6 +193,7 @@ def test_full_size_lsst_streamed():
         if True:
             with dt.Tracker.from_scene(scene) as trk:
                 trk.set_option("stream_zero_copy", int(mode))
+                trk.set_option("stream_tiles", 0)       # mode 0: whole planes in double-buffered batches
                 for j in range(cfg.n_exp):
                     trk.load_image_batch(j, flux_pool[j % POOL:j % POOL + 1], var_pool[j % POOL:j % POOL + 1])
                 snr, hits = trk.stack(el, scene.t0)

@@ -297,6 +297,7 @@ def test_streaming_batches_match_resident():
             trk.load_image_batch(half, pf[half:], pv[half:])
             trk.load_image_batch(0, pf[:half], pv[:half])
             trk.set_option("stream_zero_copy", 0)
+            trk.set_option("stream_tiles", 0)                             # whole planes, double-buffered
             snr_s, hits_s = trk.stack(el, sc.t0)
             st = trk.stats()
             assert st["streamed"] == 1 and st["n_image_batches"] == math.ceil(sc.cfg.n_exp / min(nb, 32))
@@ -440,7 +441,7 @@ def test_pinned_elements_zero_copy_matches_device_path():
                 assert s is out[0] and h is out[1]
                 res[mode] = (s.numpy().copy(), h.numpy().copy())
                 if mode == "pinned_streamed":
-                    assert trk.stats()["n_image_batches"] >= 2
+                    assert trk.stats()["streamed"] == 1
     for mode in ("pinned", "pinned_streamed"):
         assert np.array_equal(res[mode][1], res["device"][1])
         assert np.array_equal(res[mode][0], res["device"][0], equal_nan=True)
@@ -517,6 +518,7 @@ def test_streaming_zero_copy_gather_matches_copied_batches(case, expect_auto):
     for mode, want in ((0, 0), (1, 1), (-1, expect_auto)):
         with dt.Tracker.from_scene(sc, hbm_budget_bytes=2 * 20 * per_exp) as trk:
             trk.set_option("stream_zero_copy", mode)
+            trk.set_option("stream_tiles", 0)                             # the tile cache has its own test
             trk.load_image_batch(0, pf, pv)
             snr_s, hits_s = trk.stack(el, sc.t0)
             st = trk.stats()
@@ -525,6 +527,53 @@ def test_streaming_zero_copy_gather_matches_copied_batches(case, expect_auto):
             assert st["image_zero_copy"] == want, (mode, st)
         assert (st["h2d_image_bytes"] == 0) == (st["image_zero_copy"] == 1)
         assert np.array_equal(hits_s, hits_r) and np.array_equal(snr_s, snr_r), mode
+
+
+@pytest.mark.parametrize("case", ["lsst_focused", "tno_focused", "mba_focused"])
+def test_streaming_tile_cache_matches_resident(case):
+    """hits first, then only the 64 x 64-pixel tiles the hits fall on cross PCIe into a device
+    tile cache; pixels of tiles without a slot are read zero-copy.  Bit-identical to the resident run with the
+    default fetch threshold, with every touched tile fetched, with a cache of five slots (overflow -> zero-copy),
+    and with a 3 x 3 patch that crosses tile borders; fewer bytes move than the planes hold."""
+    dt = _dt()
+    sc = _scene(case)
+    cfg = sc.cfg
+    el = sc.elements()
+    flux, var = _planes(sc, cfg.variance_mode)
+    w3 = np.array([[0.1, 0.2, 0.1], [0.2, 1.0, 0.2], [0.1, 0.2, 0.1]])
+    with dt.Tracker.from_scene(sc) as trk:
+        trk.load_image_batch(0, flux, var)
+        snr_r, hits_r = trk.stack(el, sc.t0)
+        trk.set_patch(3, w3)
+        snr_p, hits_p = trk.stack(el, sc.t0)
+    pf = torch.from_numpy(flux).pin_memory()
+    pv = torch.from_numpy(var).pin_memory() if var is not None else None
+    planes = 2 if var is not None else 1
+    per_exp = flux[0].nbytes * planes
+    slot_bytes = 64 * 64 * 4 * planes
+    full = flux.nbytes * planes
+    fetched = {}
+    for label, budget, min_hits, patch in [("default", 20 * per_exp, 0, 1), ("all_tiles", 20 * per_exp, 1, 1),
+                                           ("five_slots", 5 * slot_bytes, 1, 1), ("patch3", 20 * per_exp, 4, 3)]:
+        with dt.Tracker.from_scene(sc, hbm_budget_bytes=budget) as trk:
+            trk.set_option("stream_zero_copy", 0)                         # not the pure zero-copy gather
+            trk.set_option("tile_min_hits", min_hits)
+            trk.load_image_batch(0, pf, pv)
+            if patch > 1:
+                trk.set_patch(3, w3)
+            snr_s, hits_s = trk.stack(el, sc.t0)
+            st = trk.stats()
+            snr_s2, _ = trk.stack(el, sc.t0)                              # the cache is rebuilt per call
+        assert st["streamed"] == 1 and st["image_tiles"] == 1 and st["image_zero_copy"] == 0, (label, st)
+        assert st["h2d_image_bytes"] == st["tiles_fetched"] * slot_bytes
+        want = (snr_p, hits_p) if patch > 1 else (snr_r, hits_r)
+        assert np.array_equal(hits_s, want[1]) and np.array_equal(snr_s, want[0]), label
+        assert np.array_equal(snr_s2, want[0]), label
+        fetched[label] = st["tiles_fetched"]
+    assert fetched["all_tiles"] > 0 and fetched["all_tiles"] >= fetched["default"]
+    assert fetched["five_slots"] <= 5 * ((cfg.n_exp + 511) // 512)        # the cache holds five tiles per exposure unit
+    assert fetched["all_tiles"] * slot_bytes < full, "the tile cache must move fewer bytes than the planes hold"
+    parity_record("tile_cache[%s]" % case, tiles_fetched=fetched, tile_bytes=slot_bytes, plane_bytes_total=int(full))
 
 
 @pytest.mark.parametrize("case", ["neo", "small_mba", "tno", "neo+focused", "small_mba+focused", "tno+focused"])
