@@ -54,6 +54,8 @@ def parse_args():
                     help="stop adding entries to `configs` after this many seconds (the rest is listed as skipped)")
     ap.add_argument("--count-k1", default="", help="run ONE dt_stack of this workload at a reduced orbit count "
                     "(for the ncu FP64 instruction count; see paper_2503_08854_b200/k1_counts.py) and exit")
+    ap.add_argument("--gather-real", default="", help="comma-separated workloads: kernel 3 alone on the hit list kernel 1 "
+                    "produces for the first work unit (2^20 orbits x <= 512 exposures) of each, then exit")
     ap.add_argument("--probe-random-gather", action="store_true",
                     help="run the random-gather / fetch-granularity probe (dt_probe_gather) and exit")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
@@ -248,7 +250,7 @@ def elements_device(cfg, lo, hi, dev, chunk=5_000_000):
 class Workload:
     POOL = 64          # distinct pinned exposures a beyond-HBM survey cycles through (SURVEY.md 8(d) "Host memory")
 
-    def __init__(self, dt, cfg, dev, local_rank, rank, world, flags=0):
+    def __init__(self, dt, cfg, dev, local_rank, rank, world, flags=0, same_plane=False):
         import torch
         self.dt, self.cfg, self.dev = dt, cfg, dev
 
@@ -261,7 +263,7 @@ class Workload:
         orbit_bytes = cfg.n_orbits * (48 + 36 + 12) + (6 << 30)      # elements, sums, results, hit buffers
         self.beyond_hbm = cfg.image_bytes() + orbit_bytes > free_b
         # pooled planes cannot carry per-exposure injected sources
-        self.scene = ds.build_scene(cfg, project_fn, inject=not self.beyond_hbm)
+        self.scene = ds.build_scene(cfg, project_fn, inject=not (self.beyond_hbm or same_plane))
         kw = {} if self.beyond_hbm else {"hbm_budget_bytes": cfg.image_bytes() + (1 << 30)}
         sc = self.scene
         P = min(self.POOL, cfg.n_exp)
@@ -281,6 +283,12 @@ class Workload:
                 q = j % P
                 self.trk.load_image_batch(j, fpool[q:q + 1], vpool[q:q + 1] if vpool is not None else None)
             self.keep_alive = [fpool, vpool]
+        elif same_plane:                                 # timing-only stores: every exposure carries the same seeded plane
+            f = ds.noise_plane_t(cfg, 0, dev).unsqueeze(0).contiguous()
+            v = torch.ones_like(f) if cfg.variance_mode == 1 else None
+            for j in range(cfg.n_exp):
+                self.trk.load_image_batch(j, f, v)
+            del f, v
         else:
             for j in range(cfg.n_exp):
                 f = sc.flux_plane_t(j, dev).unsqueeze(0).contiguous()
@@ -675,6 +683,22 @@ def main():
         return
 
     hbm_gbs, hbm_src = measured_hbm_peak()
+    if args.gather_real:
+        # kernel 3 alone on real hit lists: one work unit per workload; the image VALUES do not matter to the timing, so
+        # one seeded plane is registered for every exposure (resident store of the unit's exposures only)
+        regs = []
+        for name in args.gather_real.split(","):
+            cfg = ds.CONFIGS[name.split("+")[0]]
+            cfg = ds.scaled(cfg, n_orbits=min(cfg.n_orbits, UNIT_ORBITS), n_exp=min(cfg.n_exp, UNIT_EXPOSURES))
+            if name.endswith("+focused"):
+                cfg = ds.focused(cfg)
+            w = Workload(dt, cfg, dev, local_rank, 0, 1, flags=args.flags, same_plane=True)
+            u = unit_hit_list(w)
+            regs.append(gather_on_unit(w, u, hbm_gbs, flush, args.gather_reps))
+            w.close()
+        print(json.dumps({"gather_roofline": {"bound": "hbm", "kernel": "k_gather_sparse / k_gather_dense",
+                                              "peak_source": hbm_src, "regimes": regs}}))
+        return
     if args.gather_only:
         cfg = make_config(args, args.workload if args.workload != DEFAULT_WORKLOAD else "small_mba")
         w = Workload(dt, cfg, dev, local_rank, 0, 1, flags=args.flags)

@@ -209,6 +209,34 @@ int dt_threshold(dt_context *ctx, double snr_min, int32_t min_hits, int64_t max_
                  double *snr_out, int64_t *n_found);
 
 /*
+ * Exposure-sharded search.  The paper partitions the IMAGES across ranks without
+ * replication; every rank searches all orbits against its images and "the results of these computations are
+ * extremely sparse", so only the valid ones travel, asynchronously, to the process that owns the orbit
+ * (PAPER.md:141, 204-210).  Here a rank's context is created on its exposure slice; after dt_stack the per-orbit
+ * sums S = sum f/v, Wt = sum 1/v and the hit counts of that slice stay on the device, and
+ *   dt_partials_sparse    compacts, on the device, the orbits with hits > 0 into (index ascending, S, Wt, hits)
+ *                         lists -- what a rank sends; *n_found = how many there are (the first
+ *                         min(*n_found, max_out) are written; outputs live in `mem_kind` memory);
+ *   dt_partials_reset     zeroes the sums of the context;
+ *   dt_partials_add       adds one such list (indices distinct, in [0, n)) to the sums: S[i] += S_in, ...;
+ *                         calling it for the lists of ranks 0, 1, 2, ... in that order fixes the summation order
+ *                         (ascending exposure slice), so every rank computes the same bits;
+ *   dt_partials_finalize  SNR = S / sqrt(Wt) from the current sums (orbits the last dt_stack marked invalid stay
+ *                         invalid), written to snr_out / hits_out (either may be NULL) and kept for dt_topk /
+ *                         dt_threshold.
+ * The definition this reaches: S = sum over slices (in order) of the slice's sequential sum -- the plain stack up to
+ * the rounding of re-associated fp64 sums (<< the 1e-9 bar).  The exchange itself (one variable-length all-gather)
+ * is torch.distributed plumbing in the binding (paper_2503_08854_b200/sharded.py).  All need a prior dt_stack on the
+ * context (DT_ERR_STATE otherwise); n is that call's orbit count.
+ */
+int dt_partials_sparse(dt_context *ctx, int64_t max_out, int64_t *index_out, double *S_out, double *Wt_out,
+                       int32_t *hits_out, int32_t mem_kind, int64_t *n_found);
+int dt_partials_reset(dt_context *ctx);
+int dt_partials_add(dt_context *ctx, const int64_t *index, const double *S, const double *Wt, const int32_t *hits,
+                    int64_t m, int32_t mem_kind);
+int dt_partials_finalize(dt_context *ctx, double *snr_out, int32_t *hits_out, int32_t mem_kind);
+
+/*
  * dt_topk: the k largest SNR of the most recent dt_stack, SNR descending, ties by orbit index
  * ascending, over orbits with hits >= min_hits and finite SNR (Algorithm 1 `FindSignificantResults`,
  * PAPER.md:173).  index_out [k] int64, snr_out [k] fp64 are HOST pointers; *n_found = min(k, count).

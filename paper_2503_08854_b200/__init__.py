@@ -28,7 +28,8 @@ _ERR_NAMES = {-1: "DT_ERR_INVALID_ARG", -2: "DT_ERR_OOM", -3: "DT_ERR_CUDA", -4:
               -5: "DT_ERR_STATE"}
 
 EXPORTS = ["dt_create", "dt_destroy", "dt_load_image_batch", "dt_stack", "dt_stack_epochs", "dt_set_patch",
-           "dt_set_outlier_clip", "dt_threshold", "dt_topk", "dt_project",
+           "dt_set_outlier_clip", "dt_threshold", "dt_partials_sparse", "dt_partials_reset", "dt_partials_add",
+           "dt_partials_finalize", "dt_topk", "dt_project",
            "dt_gather_hits", "dt_filter_intersections", "dt_set_option", "dt_get_stats", "dt_last_error", "dt_version", "dt_fp64_peak", "dt_probe_random_gather"]
 
 
@@ -79,6 +80,10 @@ def lib():
         L.dt_set_patch.argtypes = [vp, C.c_int32, dp]
         L.dt_set_outlier_clip.argtypes = [vp, C.c_double]
         L.dt_threshold.argtypes = [vp, C.c_double, C.c_int32, C.c_int64, C.POINTER(C.c_int64), dp, C.POINTER(C.c_int64)]
+        L.dt_partials_sparse.argtypes = [vp, C.c_int64, vp, vp, vp, vp, C.c_int32, C.POINTER(C.c_int64)]
+        L.dt_partials_reset.argtypes = [vp]
+        L.dt_partials_add.argtypes = [vp, vp, vp, vp, vp, C.c_int64, C.c_int32]
+        L.dt_partials_finalize.argtypes = [vp, vp, vp, C.c_int32]
         L.dt_topk.argtypes = [vp, C.c_int32, C.c_int32, C.POINTER(C.c_int64), dp, ip]
         L.dt_project.argtypes = [vp, dp, C.c_int64, C.c_double, dp, dp, ip]
         L.dt_gather_hits.argtypes = [vp, C.c_int64, C.c_int32, C.c_int32, vp, vp, vp, C.c_int64, vp, vp, vp]
@@ -233,6 +238,62 @@ def dt_threshold(ctx, snr_min: float, min_hits: int = 0, max_out: int = 1 << 20)
                               _dp(val), C.byref(nf)), ctx)
     m = min(nf.value, max_out)
     return idx[:m].copy(), val[:m].copy(), nf.value
+
+
+def dt_partials_sparse(ctx, n: int, device=None):
+    """The orbits the context's exposure slice has hits for -> (index int64, S f64, Wt f64, hits i32), index
+    ascending; torch CUDA tensors when `device` is given, else numpy arrays."""
+    nf = C.c_int64(0)
+    _check(lib().dt_partials_sparse(ctx, 0, None, None, None, None, DT_MEM_HOST, C.byref(nf)), ctx)      # count only
+    m = nf.value
+    if device is not None:
+        import torch
+        idx = torch.empty(m, dtype=torch.int64, device=device)
+        S = torch.empty(m, dtype=torch.float64, device=device)
+        Wt = torch.empty(m, dtype=torch.float64, device=device)
+        h = torch.empty(m, dtype=torch.int32, device=device)
+        if m:
+            _check(lib().dt_partials_sparse(ctx, m, idx.data_ptr(), S.data_ptr(), Wt.data_ptr(), h.data_ptr(),
+                                            DT_MEM_DEVICE, C.byref(nf)), ctx)
+        return idx, S, Wt, h
+    idx, S, Wt, h = np.empty(m, np.int64), np.empty(m), np.empty(m), np.empty(m, np.int32)
+    if m:
+        _check(lib().dt_partials_sparse(ctx, m, idx.ctypes.data, S.ctypes.data, Wt.ctypes.data, h.ctypes.data,
+                                        DT_MEM_HOST, C.byref(nf)), ctx)
+    return idx, S, Wt, h
+
+
+def dt_partials_reset(ctx) -> None:
+    _check(lib().dt_partials_reset(ctx), ctx)
+
+
+def dt_partials_add(ctx, index, S, Wt, hits) -> None:
+    m = int(index.shape[0])
+    if m == 0:
+        return
+    pi, kind = _ptr_kind(index)
+    ps, k2 = _ptr_kind(S)
+    pw, k3 = _ptr_kind(Wt)
+    ph, k4 = _ptr_kind(hits)
+    host = (DT_MEM_HOST, DT_MEM_PINNED)
+    if not (kind == k2 == k3 == k4 or all(k in host for k in (kind, k2, k3, k4))):
+        raise ValueError("a partial-sum list must live in one kind of memory")
+    for x, want in ((index, "int64"), (S, "float64"), (Wt, "float64"), (hits, "int32")):
+        if str(x.dtype).split(".")[-1] != want or int(x.shape[0]) != m:
+            raise ValueError("partial-sum list: (int64 index, float64 S, float64 Wt, int32 hits) of equal length")
+    _check(lib().dt_partials_add(ctx, pi, ps, pw, ph, m, DT_MEM_DEVICE if kind == DT_MEM_DEVICE else DT_MEM_HOST), ctx)
+
+
+def dt_partials_finalize(ctx, n: int, device=None):
+    if device is not None:
+        import torch
+        snr = torch.empty(n, dtype=torch.float64, device=device)
+        hits = torch.empty(n, dtype=torch.int32, device=device)
+        _check(lib().dt_partials_finalize(ctx, snr.data_ptr(), hits.data_ptr(), DT_MEM_DEVICE), ctx)
+        return snr, hits
+    snr, hits = np.empty(n, np.float64), np.empty(n, np.int32)
+    _check(lib().dt_partials_finalize(ctx, snr.ctypes.data, hits.ctypes.data, DT_MEM_HOST), ctx)
+    return snr, hits
 
 
 def dt_topk(ctx, k: int, min_hits: int = 0):

@@ -94,6 +94,12 @@ struct dt_context {
     bool zero_copy_elements = true;                     // false: copy pinned elements to the device first
     std::vector<cudaEvent_t> ev_pool;                   // timing events
 
+    // scratch of the dt_partials_* calls (host-memory callers)
+    long long *d_pidx = nullptr;
+    double *d_pS = nullptr, *d_pW = nullptr;
+    int32_t *d_pc = nullptr;
+    int64_t p_cap = 0;
+    int *d_bad = nullptr;
     TopkWorkspace topk;
     dt_stats stats;
     std::string err;
@@ -150,6 +156,11 @@ void free_all(dt_context *c)
     }
     cudaFree(c->d_el);
     cudaFree(c->d_t0);
+    cudaFree(c->d_pidx);
+    cudaFree(c->d_pS);
+    cudaFree(c->d_pW);
+    cudaFree(c->d_pc);
+    cudaFree(c->d_bad);
     cudaFree(c->d_patch_w);
     cudaFree(c->d_S);
     cudaFree(c->d_Wt);
@@ -904,6 +915,106 @@ int dt_threshold(dt_context *c, double snr_min, int32_t min_hits, int64_t max_ou
     CU(c, cudaSetDevice(c->device));
     CU(c, threshold_device(c->d_snr, c->d_hits, c->n_last, snr_min, min_hits, max_out, c->topk, index_out, snr_out,
                            n_found, c->stream));
+    return DT_OK;
+}
+
+static int partial_scratch(dt_context *c, int64_t m)
+{
+    if (m <= c->p_cap && c->d_pidx) return DT_OK;
+    cudaFree(c->d_pidx); cudaFree(c->d_pS); cudaFree(c->d_pW); cudaFree(c->d_pc);
+    c->d_pidx = nullptr; c->d_pS = c->d_pW = nullptr; c->d_pc = nullptr; c->p_cap = 0;
+    const size_t k = (size_t)std::max<int64_t>(m, 1);
+    CU(c, cudaMalloc((void **)&c->d_pidx, k * 8));
+    CU(c, cudaMalloc((void **)&c->d_pS, k * 8));
+    CU(c, cudaMalloc((void **)&c->d_pW, k * 8));
+    CU(c, cudaMalloc((void **)&c->d_pc, k * 4));
+    c->p_cap = (int64_t)k;
+    return DT_OK;
+}
+
+int dt_partials_sparse(dt_context *c, int64_t max_out, int64_t *index_out, double *S_out, double *Wt_out,
+                       int32_t *cnt_out, int32_t mem_kind, int64_t *n_found)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (max_out < 0 || !n_found || !mem_kind_ok(mem_kind) || (max_out > 0 && (!index_out || !S_out || !Wt_out || !cnt_out)))
+        return fail(c, DT_ERR_INVALID_ARG, "dt_partials_sparse: bad arguments");
+    if (c->n_last < 0) return fail(c, DT_ERR_STATE, "dt_partials_sparse: no dt_stack result on the device");
+    CU(c, cudaSetDevice(c->device));
+    const int64_t n = c->n_last, cap = std::min<int64_t>(max_out, n);
+    long long *di = reinterpret_cast<long long *>(index_out);
+    double *dS = S_out, *dW = Wt_out;
+    int32_t *dc = cnt_out;
+    if (mem_kind != DT_MEM_DEVICE) {
+        int rc = partial_scratch(c, cap);
+        if (rc != DT_OK) return rc;
+        di = c->d_pidx; dS = c->d_pS; dW = c->d_pW; dc = c->d_pc;
+    }
+    CU(c, partials_sparse_device(c->d_S, c->d_Wt, c->d_cnt, n, cap, c->topk, di, dS, dW, dc, n_found, c->stream));
+    const int64_t m = std::min<int64_t>(*n_found, cap);
+    if (mem_kind != DT_MEM_DEVICE && m > 0) {
+        CU(c, cudaMemcpyAsync(index_out, di, (size_t)m * 8, cudaMemcpyDeviceToHost, c->stream));
+        CU(c, cudaMemcpyAsync(S_out, dS, (size_t)m * 8, cudaMemcpyDeviceToHost, c->stream));
+        CU(c, cudaMemcpyAsync(Wt_out, dW, (size_t)m * 8, cudaMemcpyDeviceToHost, c->stream));
+        CU(c, cudaMemcpyAsync(cnt_out, dc, (size_t)m * 4, cudaMemcpyDeviceToHost, c->stream));
+    }
+    CU(c, cudaStreamSynchronize(c->stream));
+    return DT_OK;
+}
+
+int dt_partials_reset(dt_context *c)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (c->n_last < 0) return fail(c, DT_ERR_STATE, "dt_partials_reset: no dt_stack result on the device");
+    CU(c, cudaSetDevice(c->device));
+    const size_t n = (size_t)c->n_last;
+    CU(c, cudaMemsetAsync(c->d_S, 0, n * 8, c->stream));
+    CU(c, cudaMemsetAsync(c->d_Wt, 0, n * 8, c->stream));
+    CU(c, cudaMemsetAsync(c->d_cnt, 0, n * 4, c->stream));
+    return DT_OK;
+}
+
+int dt_partials_add(dt_context *c, const int64_t *index, const double *S, const double *Wt, const int32_t *cnt,
+                    int64_t m, int32_t mem_kind)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (m < 0 || !mem_kind_ok(mem_kind) || (m > 0 && (!index || !S || !Wt || !cnt)))
+        return fail(c, DT_ERR_INVALID_ARG, "dt_partials_add: bad arguments");
+    if (c->n_last < 0) return fail(c, DT_ERR_STATE, "dt_partials_add: no dt_stack result on the device");
+    if (m == 0) return DT_OK;
+    CU(c, cudaSetDevice(c->device));
+    const long long *di = reinterpret_cast<const long long *>(index);
+    const double *dS = S, *dW = Wt;
+    const int32_t *dc = cnt;
+    if (mem_kind != DT_MEM_DEVICE) {
+        int rc = partial_scratch(c, m);
+        if (rc != DT_OK) return rc;
+        CU(c, cudaMemcpyAsync(c->d_pidx, index, (size_t)m * 8, cudaMemcpyDefault, c->stream));
+        CU(c, cudaMemcpyAsync(c->d_pS, S, (size_t)m * 8, cudaMemcpyDefault, c->stream));
+        CU(c, cudaMemcpyAsync(c->d_pW, Wt, (size_t)m * 8, cudaMemcpyDefault, c->stream));
+        CU(c, cudaMemcpyAsync(c->d_pc, cnt, (size_t)m * 4, cudaMemcpyDefault, c->stream));
+        di = c->d_pidx; dS = c->d_pS; dW = c->d_pW; dc = c->d_pc;
+    }
+    if (!c->d_bad) CU(c, cudaMalloc((void **)&c->d_bad, sizeof(int)));
+    CU(c, cudaMemsetAsync(c->d_bad, 0, sizeof(int), c->stream));
+    CU(c, partials_add_device(di, m, c->n_last, dS, dW, dc, c->d_S, c->d_Wt, c->d_cnt, c->d_bad, c->stream));
+    int bad = 0;
+    CU(c, cudaMemcpyAsync(&bad, c->d_bad, sizeof bad, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    if (bad) return fail(c, DT_ERR_INVALID_ARG, "dt_partials_add: an orbit index is outside [0, n)");
+    return DT_OK;
+}
+
+int dt_partials_finalize(dt_context *c, double *snr_out, int32_t *hits_out, int32_t mem_kind)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (!mem_kind_ok(mem_kind)) return fail(c, DT_ERR_INVALID_ARG, "dt_partials_finalize: bad arguments");
+    if (c->n_last < 0) return fail(c, DT_ERR_STATE, "dt_partials_finalize: no dt_stack result on the device");
+    CU(c, cudaSetDevice(c->device));
+    const int64_t n = c->n_last;
+    CU(c, refinalize_device(n, c->d_S, c->d_Wt, c->d_cnt, c->d_snr, c->d_hits, c->stream));
+    if (snr_out) CU(c, cudaMemcpyAsync(snr_out, c->d_snr, (size_t)n * 8, cudaMemcpyDefault, c->stream));
+    if (hits_out) CU(c, cudaMemcpyAsync(hits_out, c->d_hits, (size_t)n * 4, cudaMemcpyDefault, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
     return DT_OK;
 }
 

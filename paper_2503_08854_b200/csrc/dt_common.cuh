@@ -177,6 +177,15 @@ cudaError_t topk_device(const double *snr, const int32_t *hits, int64_t n, int32
                         int32_t min_hits, TopkWorkspace &ws, int64_t *index_out_host,
                         double *snr_out_host, int32_t *n_found, cudaStream_t stream);
 void topk_free(TopkWorkspace &ws);
+// sparse per-orbit partial sums of an exposure shard (dtrack.h dt_partials_*)
+cudaError_t partials_sparse_device(const double *S, const double *Wt, const int32_t *cnt, int64_t n, int64_t max_out,
+                                   TopkWorkspace &ws, long long *idx_out_dev, double *S_out_dev, double *Wt_out_dev,
+                                   int32_t *cnt_out_dev, int64_t *n_found, cudaStream_t stream);
+cudaError_t partials_add_device(const long long *idx, int64_t m, int64_t n, const double *S_in, const double *Wt_in,
+                                const int32_t *cnt_in, double *S, double *Wt, int32_t *cnt, int *bad_dev,
+                                cudaStream_t stream);
+cudaError_t refinalize_device(int64_t n, const double *S, const double *Wt, const int32_t *cnt, double *snr,
+                              int32_t *hits, cudaStream_t stream);
 // Threshold mode: every valid entry (finite snr >= snr_min, hits >= min_hits) in ascending index order;
 // *n_found = how many there are, the first min(*n_found, max_out) are written to the host arrays.
 cudaError_t threshold_device(const double *snr, const int32_t *hits, int64_t n, double snr_min,

@@ -239,7 +239,11 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                     // the deferred polish, then the geometric distance again from the polished state
                     // (sin E, cos E) carry 1.6e-14 of truncation per cull-quality rotation: re-synchronise
                     // them exactly once more than a few such steps have piled up
-                    if (since_sync > 6) {
+                    // (<= 1e-13 in (sin E, cos E) after six steps = 1e-7 a / rho px), and at once when some lane of the
+                    // warp is closer than a / 2 (a near-Earth pair: a / rho up to 20 would turn that into 2e-6 px)
+                    const double a_orb = sm.el[tid * 6];
+                    const bool close_pair = __any_sync(0xffffffffu, 4.0 * rho2 < a_orb * a_orb);
+                    if (since_sync > 6 || (since_sync > 0 && close_pair)) {
                         K = kepler_resync(K);
                         since_sync = 0;
                     }

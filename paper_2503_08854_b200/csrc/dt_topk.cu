@@ -463,6 +463,105 @@ cudaError_t threshold_device(const double *snr, const int32_t *hits, int64_t n, 
     return cudaStreamSynchronize(stream);
 }
 
+// ---- sparse per-orbit partial sums (exposure-sharded search; dtrack.h dt_partials_*) ---------------------------
+// The orbits a shard has hits for (cnt > 0), in ascending index order, with their sums: the same ordered
+// compaction, on the key (cnt > 0).
+__global__ void k_hit_keys(const int32_t *__restrict__ cnt, int64_t n, unsigned long long *__restrict__ keys)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) keys[i] = cnt[i] > 0 ? 1ull : 0ull;
+}
+__global__ void k_gather_partials(const long long *__restrict__ idx, int64_t m, const double *__restrict__ S,
+                                  const double *__restrict__ Wt, const int32_t *__restrict__ cnt,
+                                  double *__restrict__ S_out, double *__restrict__ Wt_out, int32_t *__restrict__ cnt_out)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < m) {
+        const long long o = idx[i];
+        S_out[i] = S[o];
+        Wt_out[i] = Wt[o];
+        cnt_out[i] = cnt[o];
+    }
+}
+// S[idx[i]] += S_in[i] ...: the indices of one list are distinct, so plain read-modify-writes; lists are added one
+// after the other in the caller's order (ascending exposure range), which fixes the summation order.
+__global__ void k_add_partials(const long long *__restrict__ idx, int64_t m, int64_t n, const double *__restrict__ S_in,
+                               const double *__restrict__ Wt_in, const int32_t *__restrict__ cnt_in,
+                               double *__restrict__ S, double *__restrict__ Wt, int32_t *__restrict__ cnt, int *bad)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < m) {
+        const long long o = idx[i];
+        if (o < 0 || o >= n) { *bad = 1; return; }
+        S[o] += S_in[i];
+        Wt[o] += Wt_in[i];
+        cnt[o] += cnt_in[i];
+    }
+}
+// SNR from the current sums; orbits marked invalid by the last dt_stack (hits < 0) stay invalid.
+__global__ void k_refinalize(int64_t n, const double *__restrict__ S, const double *__restrict__ Wt,
+                             const int32_t *__restrict__ cnt, double *__restrict__ snr, int32_t *__restrict__ hits)
+{
+    const int64_t o = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o < n && hits[o] >= 0) {
+        const int32_t c = cnt[o];
+        snr[o] = (c > 0) ? S[o] / sqrt(Wt[o]) : 0.0;
+        hits[o] = c;
+    }
+}
+
+cudaError_t partials_sparse_device(const double *S, const double *Wt, const int32_t *cnt, int64_t n, int64_t max_out,
+                                   TopkWorkspace &ws, long long *idx_out_dev, double *S_out_dev, double *Wt_out_dev,
+                                   int32_t *cnt_out_dev, int64_t *n_found, cudaStream_t stream)
+{
+    *n_found = 0;
+    if (n <= 0) return cudaSuccess;
+    const int nblocks = (int)((n + kChunk - 1) / kChunk);
+    TK_CHECK(ensure(ws.keys, ws.n_cap, n));
+    if (!ws.state) TK_CHECK(cudaMalloc((void **)&ws.state, 16 * sizeof(unsigned long long)));
+    TK_CHECK(ensure(ws.block_counts, ws.blocks_cap, (int64_t)2 * nblocks));
+    // cand_key is scratch of k_scatter: it needs max_out entries too
+    {
+        int64_t c = ws.cand_cap;
+        TK_CHECK(ensure(ws.cand_key, c, std::max<int64_t>(1, std::min<int64_t>(max_out, n))));
+        ws.cand_cap = c;
+        // cand_idx is NOT used: the indices go straight to the caller's buffer
+    }
+    TK_CHECK(cudaMemsetAsync(ws.state, 0, 16 * sizeof(unsigned long long), stream));      // T = 0, no ties
+    k_hit_keys<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(cnt, n, ws.keys);
+    k_count<<<nblocks, kThreads, 0, stream>>>(ws.keys, n, ws.state, ws.block_counts);
+    k_scan<<<1, 1024, 0, stream>>>(ws.block_counts, nblocks, ws.state);
+    k_scatter<<<nblocks, kThreads, 0, stream>>>(ws.keys, n, ws.state, ws.block_counts, ws.cand_key, idx_out_dev,
+                                                (unsigned long long)max_out);
+    TK_CHECK(cudaGetLastError());
+    unsigned long long st[8];
+    TK_CHECK(cudaMemcpyAsync(st, ws.state, sizeof st, cudaMemcpyDeviceToHost, stream));
+    TK_CHECK(cudaStreamSynchronize(stream));
+    *n_found = (int64_t)st[7];
+    const int64_t m = std::min<int64_t>(*n_found, max_out);
+    if (m > 0)
+        k_gather_partials<<<(unsigned)((m + 255) / 256), 256, 0, stream>>>(idx_out_dev, m, S, Wt, cnt, S_out_dev,
+                                                                          Wt_out_dev, cnt_out_dev);
+    return cudaGetLastError();
+}
+
+cudaError_t partials_add_device(const long long *idx, int64_t m, int64_t n, const double *S_in, const double *Wt_in,
+                                const int32_t *cnt_in, double *S, double *Wt, int32_t *cnt, int *bad_dev,
+                                cudaStream_t stream)
+{
+    if (m <= 0) return cudaSuccess;
+    k_add_partials<<<(unsigned)((m + 255) / 256), 256, 0, stream>>>(idx, m, n, S_in, Wt_in, cnt_in, S, Wt, cnt, bad_dev);
+    return cudaGetLastError();
+}
+
+cudaError_t refinalize_device(int64_t n, const double *S, const double *Wt, const int32_t *cnt, double *snr,
+                              int32_t *hits, cudaStream_t stream)
+{
+    if (n <= 0) return cudaSuccess;
+    k_refinalize<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(n, S, Wt, cnt, snr, hits);
+    return cudaGetLastError();
+}
+
 void topk_free(TopkWorkspace &ws)
 {
     cudaFree(ws.keys);

@@ -187,3 +187,76 @@ def test_patch_through_the_zero_copy_gather():
             snr, hits = trk.stack(el, sc.t0)
             assert trk.stats()["image_zero_copy"] == zero_copy
             _compare(snr, hits, ref, "patch 3 clip 3 streamed zero_copy=%d" % zero_copy)
+
+
+def test_exposure_sharded_partial_sums():
+    """SURVEY 8(f) NEXT-4 on one GPU: two contexts on the two halves of the exposures stand for two ranks (no rank
+    waits on another: the lists are handed over in-process; the all-gather itself is tested with gloo in
+    tests/test_sharded_gloo.py).  Each compacts its sparse per-orbit sums on the device; adding the lists in rank order
+    on either context gives, bit for bit, the oracle's sums of the two slices added in that order, the plain stack's
+    hit counts, and its SNR to the rounding of a re-associated sum; top-k and threshold see the merged result."""
+    dt = _dt()
+    from paper_2503_08854_b200.sharded import exposure_slices
+    base, kw = CASES["mba_scalar_var"]
+    sc, flux, var = _scene(base, **kw)
+    el = sc.elements().copy()
+    el[3, 1] = 1.5                                               # one invalid orbit
+    n, N = el.shape[0], sc.cfg.n_exp
+    sv = oracle.Survey.from_scene(sc)
+    full = oracle.stack(sv, list(flux), None, el, sc.t0)
+    slices = exposure_slices(N, 2)
+    ref_S, ref_W, ref_h = np.zeros(n), np.zeros(n), np.zeros(n, np.int64)
+    for lo, hi in slices:                                        # the sharded definition, from the oracle
+        sub = oracle.Survey(sc.t[lo:hi], sc.obs_ecl[lo:hi], sc.ra0[lo:hi], sc.dec0[lo:hi], sc.cfg.width, sc.cfg.height,
+                            sc.pixel_scale, sc.gm, sc.c, sc.obliquity, 0, sc.var_scalar[lo:hi])
+        r = oracle.stack(sub, list(flux[lo:hi]), None, el, sc.t0)
+        ok = r["hits"] > 0
+        ref_S[ok] += r["S"][ok]
+        ref_W[ok] += r["Wt"][ok]
+        ref_h[ok] += r["hits"][ok]
+    el_dev = torch.from_numpy(el).cuda()
+    trks, lists = [], []
+    try:
+        for (lo, hi) in slices:
+            t = dt.Tracker(sc.t[lo:hi], sc.obs_ecl[lo:hi], sc.ra0[lo:hi], sc.dec0[lo:hi], sc.cfg.width, sc.cfg.height,
+                           sc.pixel_scale, gm=sc.gm, c=sc.c, obliquity=sc.obliquity, variance_mode=0,
+                           var_scalar=sc.var_scalar[lo:hi])
+            t.load_image_batch(0, flux[lo:hi])
+            t.stack(el_dev, sc.t0)
+            trks.append(t)
+            lists.append(dt.dt_partials_sparse(t.ctx, n, device=el_dev.device))
+        assert all(0 < int(p[0].numel()) < n for p in lists), "sparse lists"
+        assert all(bool((p[0][1:] > p[0][:-1]).all()) for p in lists), "index ascending"
+        results = []
+        for t in trks:                                           # every "rank" merges all lists in rank order
+            dt.dt_partials_reset(t.ctx)
+            for part in lists:
+                dt.dt_partials_add(t.ctx, *part)
+            snr, hits = dt.dt_partials_finalize(t.ctx, n, device=el_dev.device)
+            results.append((snr.cpu().numpy(), hits.cpu().numpy()))
+        assert np.array_equal(results[0][0], results[1][0], equal_nan=True) and np.array_equal(results[0][1], results[1][1])
+        snr, hits = results[0]
+        clean = full["nflag"] == 0
+        assert hits[3] == -1 and np.isnan(snr[3])
+        assert np.array_equal(hits[clean], full["hits"][clean])
+        want = np.where(ref_h > 0, ref_S / np.sqrt(np.where(ref_W > 0, ref_W, 1.0)), 0.0)
+        same = clean & (hits == ref_h) & (hits >= 0)
+        assert same.sum() > n // 2 and np.array_equal(snr[same], want[same]), "the sharded definition, bit for bit"
+        assert np.all(np.abs(snr - full["snr"])[clean & (hits >= 0)] <= 1e-9 * np.maximum(np.abs(full["snr"]), 1e-3)[clean & (hits >= 0)])
+        idx, val = trks[0].topk(5, min_hits=1)
+        widx, wval = oracle.topk(snr, hits, 5, 1)
+        assert np.array_equal(idx, widx) and np.array_equal(val, wval)
+        # host lists work too, and a bad index is refused
+        dt.dt_partials_reset(trks[0].ctx)
+        for part in lists:
+            dt.dt_partials_add(trks[0].ctx, *[x.cpu().numpy() for x in part])
+        snr_h, hits_h = dt.dt_partials_finalize(trks[0].ctx, n)
+        assert np.array_equal(snr_h, snr, equal_nan=True) and np.array_equal(hits_h, hits)
+        with pytest.raises(dt.DtError):
+            dt.dt_partials_add(trks[0].ctx, np.array([n], np.int64), np.ones(1), np.ones(1), np.ones(1, np.int32))
+        parity_record("next[sharded x2]", orbits=n, flagged_orbits=int((~clean).sum()), hits=int(ref_h.sum()),
+                      snr_bit_identical=int(same.sum()), compared=int(same.sum()),
+                      list_lengths=[int(p[0].numel()) for p in lists])
+    finally:
+        for t in trks:
+            t.close()
