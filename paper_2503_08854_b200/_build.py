@@ -36,30 +36,38 @@ def _stale() -> bool:
     return os.path.getmtime(LIB) < max(os.path.getmtime(d) for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not _stale():
+LIB_BOUNDS = os.path.join(HERE, "libdtrack_bounds.so")
+
+
+def build(force: bool = False, verbose: bool = False, bounds: bool = False) -> str:
+    """bounds=True: the debug build with device-side bounds checks (-DDT_BOUNDS_CHECK) -> libdtrack_bounds.so; load it
+    with DTRACK_LIB=<path> (the binding honours it)."""
+    if not bounds and not force and not _stale():
         return LIB
     nvcc = _nvcc()
     objs = []
     log = []
+    lib = LIB_BOUNDS if bounds else LIB
     for src in SOURCES:
-        obj = os.path.join(CSRC, src.replace(".cu", ".o"))
-        cmd = [nvcc] + NVCC_FLAGS + ["-I", INCLUDE, "-c", os.path.join(CSRC, src), "-o", obj]
+        obj = os.path.join(CSRC, src.replace(".cu", ".bounds.o" if bounds else ".o"))
+        cmd = [nvcc] + NVCC_FLAGS + (["-DDT_BOUNDS_CHECK"] if bounds else []) + \
+              ["-I", INCLUDE, "-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         log.append(r.stderr)
         if r.returncode != 0:
             raise RuntimeError("nvcc failed on %s:\n%s\n%s" % (src, r.stdout, r.stderr))
         objs.append(obj)
-    cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs
+    cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", lib] + objs
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError("link failed:\n%s\n%s" % (r.stdout, r.stderr))
-    with open(os.path.join(CSRC, "ptxas.log"), "w") as f:
-        f.write("\n".join(log))
+    if not bounds:
+        with open(os.path.join(CSRC, "ptxas.log"), "w") as f:
+            f.write("\n".join(log))
     if verbose:
         print("\n".join(log))
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, bounds="--bounds" in sys.argv))

@@ -301,7 +301,11 @@ int ensure_store(dt_context *c)
 
 extern "C" {
 
-const char *dt_version(void) { return "dtrack-b200 0.1 sm_100a"; }
+#ifdef DT_BOUNDS_CHECK
+const char *dt_version(void) { return "dtrack-b200 0.2 sm_100a +bounds"; }
+#else
+const char *dt_version(void) { return "dtrack-b200 0.2 sm_100a"; }
+#endif
 
 const char *dt_last_error(const dt_context *ctx) { return ctx ? ctx->err.c_str() : g_static_err; }
 
@@ -468,6 +472,9 @@ static int propagate_mode(const dt_context *c)
 
 static void fill_gather_ext(const dt_context *c, GatherParams &g)
 {
+    g.tile_capacity = c->tile_capacity;
+    g.offsets_cap = g.offsets == c->d_offsets ? c->off_cap : (int64_t)1 << 40;   // dt_gather_hits: the caller's list
+    g.bounds = c->d_counters + 7;
     g.patch = c->patch;
     g.patch_w = c->d_patch_w;
     g.clip = c->clip;
@@ -489,6 +496,7 @@ static void fill_common(const dt_context *c, PropagateParams &p, double t0)
     p.H = (double)c->H;
     p.width = c->W;
     p.tan_fov = c->tan_fov;
+    p.offsets_cap = c->off_cap;
 }
 
 static int32_t pick_groups_per_split(int64_t n_orbits, int32_t n_exp)
@@ -777,6 +785,8 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
                 t.var_ptrs = (c->var_mode == 1) ? c->d_var_ptrs : nullptr;
                 t.tile_buf = c->tile_buf;
                 t.slot_floats = c->slot_floats;
+                t.offsets_cap = c->off_cap;
+                t.bounds = c->d_counters + 7;
                 CU(c, launch_tiles(t, c->sm_count, c->stream));
                 g.tile_slot = c->tile_slot;
                 g.tile_buf = c->tile_buf;
@@ -857,6 +867,8 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
     st.cold_solves = (int64_t)hc[2];
     st.substep_solves = (int64_t)hc[4];
     st.invalid_orbits = (int64_t)hc[5];
+    if (hc[7] != 0)
+        return fail(c, DT_ERR_CUDA, "bounds-check build: %llu out-of-bounds indices were caught on the device", hc[7]);
     st.launches = st.propagate_launches + st.gather_launches + 1;
     c->n_last = n;
     return DT_OK;
@@ -1131,7 +1143,19 @@ int dt_gather_hits(dt_context *c, int64_t n, int32_t first_exposure, int32_t n_g
     g.n_exp_store = c->N;
     g.sm_count = c->sm_count;
     fill_gather_ext(c, g);
+    g.offsets_cap = n_hits;
+#ifdef DT_BOUNDS_CHECK
+    CU(c, cudaMemsetAsync(c->d_counters + 7, 0, sizeof(unsigned long long), c->stream));
+#endif
     CU(c, launch_gather(g, c->device, c->stream));
+#ifdef DT_BOUNDS_CHECK
+    {
+        unsigned long long bad = 0;
+        CU(c, cudaMemcpyAsync(&bad, c->d_counters + 7, sizeof bad, cudaMemcpyDeviceToHost, c->stream));
+        CU(c, cudaStreamSynchronize(c->stream));
+        if (bad) return fail(c, DT_ERR_CUDA, "bounds-check build: %llu out-of-bounds indices were caught on the device", bad);
+    }
+#endif
     return DT_OK;
 }
 

@@ -5,6 +5,16 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+// Debug build (-DDT_BOUNDS_CHECK; `python -m paper_2503_08854_b200._build --bounds` -> libdtrack_bounds.so):
+// every data-dependent index of kernels 1 - 3 and of the tile kernels is checked on the device; a violation is
+// counted (counters[7]) and skipped, and the call that ran the kernel fails with DT_ERR_CUDA.  compute-sanitizer
+// is closed on the GPU pool this was developed on (profiles/r2_memcheck.md); this is its stand-in.
+#ifdef DT_BOUNDS_CHECK
+#define DT_IN_BOUNDS(cond, ctr) ((cond) ? true : ((ctr) ? (atomicAdd((ctr), 1ull), false) : false))
+#else
+#define DT_IN_BOUNDS(cond, ctr) true
+#endif
+
 namespace dt {
 
 // ---- per-exposure constant record ("a few hundred bytes of data for each image") ---
@@ -50,7 +60,8 @@ struct PropagateParams {
     uint32_t *mask;             // [n_groups][n_pad]
     unsigned long long *base;   // [n_groups][n_pad/32]
     uint32_t *offsets;          // [capacity]
-    unsigned long long *counters;  // [0] unit hit allocator, [1] refined pairs, [2] cold solves, [3] hits
+    int64_t offsets_cap;        // entries `offsets` can hold (bounds-check build)
+    unsigned long long *counters;  // [0] unit hit allocator, [1] refined pairs, [2] cold solves, [3] hits, [7] bounds violations
     // dense debug outputs (dt_project), NULL on the timed path
     double *radec, *xy;         // [n][n_exp][2]
     int32_t *pix;               // [n][n_exp][2]
@@ -107,6 +118,9 @@ struct GatherParams {
     int64_t slot_floats;
     int32_t ts_log2, tiles_x, tiles_per_plane;
     int32_t tile_e0;            // absolute exposure of row 0 of tile_slot
+    int32_t tile_capacity;      // slots of tile_buf (bounds-check build)
+    int64_t offsets_cap;        // entries `offsets` holds (bounds-check build)
+    unsigned long long *bounds; // violation counter of the bounds-check build (NULL: not counted)
 };
 
 // ---- tiled image cache of the streaming mode (dt_tiles.cu) -------------------------------------------------------
@@ -129,6 +143,8 @@ struct TileParams {
     const float *const *var_ptrs;    // NULL in scalar-variance mode
     float *tile_buf;
     int64_t slot_floats;
+    int64_t offsets_cap;        // bounds-check build
+    unsigned long long *bounds;
 };
 cudaError_t launch_tiles(const TileParams &t, int sm_count, cudaStream_t stream);
 

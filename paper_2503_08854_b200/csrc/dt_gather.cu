@@ -38,8 +38,10 @@ __device__ __forceinline__ bool load_pixel_tiled(const GatherParams &p, int64_t 
 {
     const uint32_t y = a / (uint32_t)p.width, x = a - y * (uint32_t)p.width;
     const int tile = (int)(y >> p.ts_log2) * p.tiles_x + (int)(x >> p.ts_log2);
+    if (!DT_IN_BOUNDS(j >= p.tile_e0 && j - p.tile_e0 < 512 && tile < p.tiles_per_plane, p.bounds)) return false;
     const int32_t s = p.tile_slot[(j - p.tile_e0) * p.tiles_per_plane + tile];
     if (s < 0) return false;
+    if (!DT_IN_BOUNDS(s < p.tile_capacity, p.bounds)) return false;
     const uint32_t m = (1u << p.ts_log2) - 1u;
     const uint32_t k = ((y & m) << p.ts_log2) + (x & m);
     const float *t = p.tile_buf + (int64_t)s * p.slot_floats;
@@ -127,8 +129,9 @@ __global__ void __launch_bounds__(kSparseThreads) k_gather_sparse(const GatherPa
                 bits &= bits - 1u;
                 const uint32_t cj = __shfl_sync(0xffffffffu, col, jj);
                 const uint32_t pj = __shfl_sync(0xffffffffu, pre, jj);
-                if (have) {
+                if (have && DT_IN_BOUNDS((int64_t)(pj + __popc(cj & lt)) < p.offsets_cap, p.bounds)) {
                     const uint32_t off = p.offsets[pj + __popc(cj & lt)] & kOffsetMask;
+                    if (!DT_IN_BOUNDS((int64_t)off < p.plane && j0 + jj < p.n_exp_store, p.bounds)) continue;
                     const int iy = (int)(off / (uint32_t)p.width), ix = (int)(off - (uint32_t)iy * (uint32_t)p.width);
                     const int64_t j = j0 + jj;
                     const double v_scalar = PLANE_VAR ? 0.0 : p.exp_all[j].var;
@@ -174,7 +177,11 @@ __global__ void __launch_bounds__(kSparseThreads) k_gather_sparse(const GatherPa
                 idx[q] = pj + __popc(cj & lt);
             }
 #pragma unroll
-            for (int q = 0; q < 4; ++q) off[q] = have[q] ? (p.offsets[idx[q]] & kOffsetMask) : 0u;
+            for (int q = 0; q < 4; ++q) {
+                have[q] = have[q] && DT_IN_BOUNDS((int64_t)idx[q] < p.offsets_cap, p.bounds);
+                off[q] = have[q] ? (p.offsets[idx[q]] & kOffsetMask) : 0u;
+                have[q] = have[q] && DT_IN_BOUNDS((int64_t)off[q] < p.plane && j0 + jj[q] < p.n_exp_store, p.bounds);
+            }
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 f[q] = 0.f;

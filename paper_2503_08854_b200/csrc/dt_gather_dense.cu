@@ -130,9 +130,10 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherCtasPerSm) k_gather_den
             for (int t = 0; t < kMaxTilesPerWarp; ++t) {
                 const bool h = (bits[t] >> jj) & 1u;
                 const unsigned hm = __ballot_sync(0xffffffffu, h);
-                off[t] = h ? (p.offsets[cur[t] + __popc(hm & lt)] & kOffsetMask) : 0u;
+                const bool hb = h && DT_IN_BOUNDS((int64_t)(cur[t] + __popc(hm & lt)) < p.offsets_cap, p.bounds);
+                off[t] = hb ? (p.offsets[cur[t] + __popc(hm & lt)] & kOffsetMask) : 0u;
                 cur[t] += __popc(hm);
-                mine |= h ? (1u << t) : 0u;
+                mine |= (hb && DT_IN_BOUNDS((int64_t)off[t] < p.plane, p.bounds)) ? (1u << t) : 0u;
             }
             // ---- is this warp's hit set spread over the plane?  (predictor for the prefetch above;
             // re-evaluated on the first exposure of every group only: the reuse regime is issue-bound) ----

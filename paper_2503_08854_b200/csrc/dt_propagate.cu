@@ -314,7 +314,8 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 // ---- cull + compaction, stage 1: ballot-compact this exposure's hits ----
                 const unsigned hm = __ballot_sync(0xffffffffu, hit);
                 if (hm) {
-                    if (hit) {
+                    if (hit && DT_IN_BOUNDS(run + __popc(hm & ((1u << lane) - 1u)) < kGroup * 32 &&
+                                                (int64_t)iy * p.width + ix < (int64_t)p.W * (int64_t)p.H, p.counters + 7)) {
                         sm.stage[warp][run + __popc(hm & ((1u << lane) - 1u))] =
                             ((uint32_t)jj << kOffsetBits) | ((uint32_t)iy * (uint32_t)p.width + (uint32_t)ix);
                         bits |= 1u << jj;
@@ -334,7 +335,8 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 b0 = __shfl_sync(0xffffffffu, b0, 0);
                 __syncwarp();
                 uint32_t *dst = p.offsets + b0;
-                for (int k = lane; k < run; k += 32) dst[k] = sm.stage[warp][k];
+                if (DT_IN_BOUNDS((int64_t)b0 + run <= p.offsets_cap, p.counters + 7))
+                    for (int k = lane; k < run; k += 32) dst[k] = sm.stage[warp][k];
             }
             const int64_t opad = (int64_t)blockIdx.x * kTileOrbits + tid;
             if (opad < p.n_pad) {

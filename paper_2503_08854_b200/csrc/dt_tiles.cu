@@ -38,8 +38,11 @@ __global__ void __launch_bounds__(kTileThreads) k_tile_count(const TileParams t)
     if (m == 0) return;
     const uint32_t blk0 = (uint32_t)t.base[g * n_tiles + wt];
     for (int k = lane; k < m; k += 32) {
+        if (!DT_IN_BOUNDS((int64_t)blk0 + k < t.offsets_cap, t.bounds)) continue;
         const uint32_t e = t.offsets[blk0 + k];
         const uint32_t off = e & kOffsetMask;
+        if (!DT_IN_BOUNDS((int64_t)off < (int64_t)t.width * t.height && g * kGroup + (e >> kOffsetBits) < (uint32_t)t.n_exp, t.bounds))
+            continue;
         const int y = (int)(off / (uint32_t)t.width), x = (int)(off - (uint32_t)y * (uint32_t)t.width);
         const int tile = (y >> t.ts_log2) * t.tiles_x + (x >> t.ts_log2);
         const int64_t row = g * kGroup + (e >> kOffsetBits);                         // exposure within the unit
@@ -60,7 +63,7 @@ __global__ void __launch_bounds__(kTileThreads) k_tile_assign(const TileParams t
     if (s >= (unsigned)t.capacity) return;               // cache full: this tile stays zero-copy
     t.tile_slot[i] = (int32_t)s;
     const unsigned q = atomicAdd(t.alloc + 1, 1u);
-    t.fetch_list[q] = make_uint2((unsigned)i, s);
+    if (DT_IN_BOUNDS(q < (unsigned)t.capacity, t.bounds)) t.fetch_list[q] = make_uint2((unsigned)i, s);
 }
 
 // ---- 4: host plane -> tile slot.  One CTA per queued tile (grid-stride), 64 threads per 256-B row segment ----

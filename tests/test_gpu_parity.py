@@ -401,6 +401,45 @@ def test_gather_hits_entry_matches_definition(schedule, var_mode):
     assert np.array_equal(dS.cpu().numpy(), S) and np.array_equal(dW.cpu().numpy(), Wt)
 
 
+def test_bounds_check_build_catches_a_corrupt_hit_list():
+    """compute-sanitizer is closed on the GPU pool (profiles/r2_memcheck.md); its stand-in is the -DDT_BOUNDS_CHECK
+    build (python -m paper_2503_08854_b200._build --bounds; DTRACK_LIB=.../libdtrack_bounds.so pytest -m gpu): every
+    data-dependent index is checked on the device.  With that build loaded, a hit list whose entry points outside the
+    plane, or whose block base points outside the list, must be refused; with the normal build the test only checks
+    that a well-formed list passes."""
+    dt = _dt()
+    N, H, W, n = 32, 64, 64, 64
+    t = np.linspace(0, 5, N)
+    flux = np.ones((N, H, W), np.float32)
+    mask = np.zeros((1, n), np.uint32)
+    mask[0, 5] = 1                                        # orbit 5 hits exposure 0
+    base = np.zeros((1, n // 32), np.uint64)
+    bounds = "+bounds" in dt.dt_version()
+    with dt.Tracker(t, ds.observer_ecliptic(t), np.zeros(N), np.zeros(N), W, H, ds.PIXEL_SCALE, variance_mode=0,
+                    var_scalar=np.ones(N)) as trk:
+        trk.load_image_batch(0, flux)
+        trk.set_option("gather_schedule", 0)
+
+        def run(entry, base0=0):
+            b = base.copy()
+            b[0, 0] = base0
+            dS = torch.zeros(n, dtype=torch.float64, device="cuda")
+            dW = torch.zeros(n, dtype=torch.float64, device="cuda")
+            dc = torch.zeros(n, dtype=torch.int32, device="cuda")
+            trk.gather_hits(n, 0, 1, torch.from_numpy(mask.view(np.int32)).cuda(), torch.from_numpy(b.view(np.int64)).cuda(),
+                            torch.tensor([entry], dtype=torch.int32).cuda(), 1, dS, dW, dc)
+            torch.cuda.synchronize()
+            return int(dc.sum())
+
+        assert run(7 * W + 3) == 1
+        if bounds:
+            with pytest.raises(dt.DtError):
+                run(H * W + 10)                           # pixel offset outside the plane
+            with pytest.raises(dt.DtError):
+                run(7 * W + 3, base0=1000)                # block base outside the list
+    print("library:", dt.dt_version())
+
+
 def test_fp64_peak_probe_runs():
     dt = _dt()
     tf = dt.dt_fp64_peak(0)
