@@ -28,7 +28,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 TABLE = os.path.join(HERE, "k1_fp64_counts.json")
-KERNEL_SOURCES = ["dt_propagate.cu", "dt_orbit.cuh", "dt_common.cuh", "dt_tma.cuh"]
+KERNEL_SOURCES = ["dt_propagate.cu", "dt_orbit.cuh", "dt_k1.cuh", "dt_tma.cuh"]
 
 
 def source_hash() -> str:
