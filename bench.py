@@ -733,6 +733,7 @@ def main():
     n_main = w.n
     topk_ms = {}
     if rank == 0:                                      # device top-k / threshold over the step's per-orbit SNR
+        w.trk.stack(w.el_dev, w.scene.t0)              # (the real-hit-list roofline ran dt_filter_intersections since)
         for k in (64, 4096):
             w.trk.topk(k, min_hits=1)
             t0 = time.perf_counter()

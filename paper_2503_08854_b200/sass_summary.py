@@ -79,7 +79,7 @@ def main():
     px = ptxas_info()
     print("| kernel | regs | static smem B | spill st/ld B | SASS instr. | " + " | ".join(c for c, _ in CLASSES) + " |")
     print("|---|---|---|---|---|" + "---|" * len(CLASSES))
-    for obj in sorted(f for f in os.listdir(CSRC) if f.endswith(".o")):
+    for obj in sorted(f for f in os.listdir(CSRC) if f.endswith(".o") and not f.endswith(".bounds.o")):
         for name, ins in kernels_of(os.path.join(CSRC, obj)).items():
             counts = []
             for _c, rx in CLASSES:
