@@ -176,11 +176,11 @@ def run_reference(args, cfg, rank: int):
     n_orb = int(min(cfg.n_orbits, max(2000, rate0 * 2.0 / n_exp_s)))
     for _ in range(args.warmup):
         oracle_sample_rate(cfg, n_orb, n_exp_s)
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        oracle_sample_rate(cfg, n_orb, n_exp_s)
-    dt_s = (time.perf_counter() - t0) / max(args.steps, 1)
-    value = n_orb * n_exp_s / dt_s
+    rates = []
+    for _ in range(args.steps):                      # each step: oracle.stack on the sample (input generation untimed)
+        rates.append(oracle_sample_rate(cfg, n_orb, n_exp_s)[0])
+    value = float(np.mean(rates)) if rates else 0.0
+    dt_s = n_orb * n_exp_s / value if value else 0.0
     sample = "oracle.stack, first %d orbits x first %d exposures of %s per step" % (n_orb, n_exp_s, cfg.name)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt_s * 1e3, "higher_is_better": True,
