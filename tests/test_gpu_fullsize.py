@@ -87,6 +87,27 @@ def _check_sample(cfg, scene, plane_of, snr, hits, sample, label):
     return rep
 
 
+def _check_block_hit_counts(cfg, scene, hits, label, n_block=20000, lo=None):
+    """A contiguous block of orbits, not chosen by the GPU's result: the oracle's projection gives every orbit's
+    footprint hits over ALL exposures (the synthetic images carry no masked pixel, so that is the hit count); the
+    GPU's counts must equal them exactly off the guard band and differ by at most the flagged pairs on it.  An orbit
+    the GPU wrongly reports with zero (or too many) hits cannot hide behind the random sample."""
+    lo = (cfg.n_orbits // 3) if lo is None else lo
+    hi = min(cfg.n_orbits, lo + n_block)
+    el = ds.elements(cfg, lo, hi)
+    pr = oracle.project(oracle.Survey.from_scene(scene), el, scene.t0)
+    want = (pr["pix"][..., 0] >= 0).sum(1)
+    nflag = pr["flag"].astype(np.int64).sum(1)
+    got = hits[lo:hi]
+    clean = nflag == 0
+    assert np.array_equal(got[clean], want[clean]), (label, np.flatnonzero(got[clean] != want[clean])[:10] + lo)
+    assert (np.abs(got - want) <= nflag).all(), label
+    rep = dict(block=[int(lo), int(hi)], pairs=int((hi - lo) * cfg.n_exp), oracle_hits=int(want.sum()),
+               flagged_pairs=int(nflag.sum()), hit_count_mismatch_on_flagged=int((got != want).sum()))
+    parity_record("fullsize_block[%s]" % label, **rep)
+    return rep
+
+
 def _pick_sample(scene, hits_dev, n):
     rng = np.random.default_rng(12345)
     rand = rng.integers(0, n, N_RANDOM)
@@ -150,6 +171,10 @@ def test_full_size_resident(name):
             return fl, (np.full_like(fl, np.float32(scene.var_scalar[j])) if cfg.variance_mode == 1 else None)
 
         rep = _check_sample(cfg, scene, plane_of, snr_h, hits_h, sample, name)
+        blk = _check_block_hit_counts(cfg, scene, hits_h, name)
+        if name.endswith("+focused"):
+            assert blk["oracle_hits"] > 1000, "vacuous block"
+        print(name, blk)
         print(name, "pairs %.3g hits %d ms %.1f" % (cfg.pairs, st["hits"], st["ms_total"]), rep)
         if name.endswith("+focused"):
             assert rep["with_hits"] > 0
@@ -214,6 +239,7 @@ def test_full_size_lsst_streamed():
         return flux_pool[j % POOL].numpy(), var_pool[j % POOL].numpy()
 
     rep = _check_sample(cfg, scene, plane_of, snr_h, hits_h, sample, "lsst streamed")
+    _check_block_hit_counts(cfg, scene, hits_h, "lsst streamed", n_block=10000)
     gbs = st["h2d_image_bytes"] / (st["ms_total"] * 1e-3) * 1e-9
     print("lsst streamed: pairs %.3g hits %d ms %.0f (%.1f GB/s host->device); zero-copy gather: ms %.0f (%.3g pairs/s)" %
           (cfg.pairs, st["hits"], st["ms_total"], gbs, results["-1"][2]["ms_total"],
