@@ -75,12 +75,14 @@ __device__ __forceinline__ Orbit orbit_setup(const double el_in[6], double gm, d
     const double vmax = sqrt(gm / a * (1.0 + e) / (1.0 - e));
     const double th = atan(tan_fov) * 1.01 + 1.05 * asin(fmin(vmax * inv_c, 1.0)) + 1.4e-4;
     const double cth = (th < 1.5) ? cos(th) : 0.0;
-    o.cos2_cull = (th < 1.5) ? cth * cth : -1.0;  // -1: cone test disabled (always refine)
+    o.cos2_cull = (th < 1.5) ? cth * cth : 0.0;
     // The cull may run on an UNPOLISHED order-2 Kepler state, off by <= 6e-6 rad in E (k_propagate), i.e.
     // by <= 6e-6 a AU in position (|dr/dE| <= a) and 6e-6 a / rho in direction: 1e-4 rad of the slack
     // above are reserved for it, which holds for rho >= 0.06 a; closer pairs (and anything inside
     // 0.1 AU) are refined unconditionally.
-    o.rho2_close = fmax(0.01, 0.0036 * a * a);
+    // (a cone wider than 1.5 rad is no cone: such an orbit is refined everywhere -- through an infinite rho2_close,
+    // which costs the hot loop no compare of its own)
+    o.rho2_close = (th < 1.5) ? fmax(0.01, 0.0036 * a * a) : INFINITY;
     return o;
 }
 

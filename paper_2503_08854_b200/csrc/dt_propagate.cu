@@ -222,7 +222,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
             if (PRECULL) {
                 // conservative cone test on the GEOMETRIC direction (see orbit_setup)
                 const double D0 = fma(dx0, x.tx, fma(dy0, x.ty, dz0 * x.tz));
-                near = !(D0 * D0 < o.cos2_cull * rho2) && (D0 > 0.0 || o.cos2_cull < 0.0);
+                near = !(D0 * D0 < o.cos2_cull * rho2) && D0 > 0.0;
                 // always refine close objects: there the error of the unpolished state could move the
                 // direction by more than the cone's slack (and rho2 ~ 0 must not cull)
                 near = near || !(rho2 > o.rho2_close);
@@ -287,6 +287,21 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                     ix = __double2int_rz(xh);
                     iy = __double2int_rz(yh);
                 }
+                if (!DENSE) {
+                    // ---- cull + compaction, stage 1: ballot-compact this exposure's hits (only a warp that refined
+                    // can have any) ----
+                    const unsigned hm = __ballot_sync(0xffffffffu, hit);
+                    if (hm) {
+                        if (hit && DT_IN_BOUNDS(run + __popc(hm & ((1u << lane) - 1u)) < kGroup * 32 &&
+                                                    (int64_t)iy * p.width + ix < (int64_t)p.W * (int64_t)p.H, p.counters + 7)) {
+                            sm.stage[warp][run + __popc(hm & ((1u << lane) - 1u))] =
+                                ((uint32_t)jj << kOffsetBits) | ((uint32_t)iy * (uint32_t)p.width + (uint32_t)ix);
+                            bits |= 1u << jj;
+                            cnt += 1;
+                        }
+                        run += __popc(hm);
+                    }
+                }
             }
             if (DENSE) {
                 if (in_range) {
@@ -309,19 +324,6 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                         p.pix[k] = ix;
                         p.pix[k + 1] = iy;
                     }
-                }
-            } else {
-                // ---- cull + compaction, stage 1: ballot-compact this exposure's hits ----
-                const unsigned hm = __ballot_sync(0xffffffffu, hit);
-                if (hm) {
-                    if (hit && DT_IN_BOUNDS(run + __popc(hm & ((1u << lane) - 1u)) < kGroup * 32 &&
-                                                (int64_t)iy * p.width + ix < (int64_t)p.W * (int64_t)p.H, p.counters + 7)) {
-                        sm.stage[warp][run + __popc(hm & ((1u << lane) - 1u))] =
-                            ((uint32_t)jj << kOffsetBits) | ((uint32_t)iy * (uint32_t)p.width + (uint32_t)ix);
-                        bits |= 1u << jj;
-                        cnt += 1;
-                    }
-                    run += __popc(hm);
                 }
             }
         }
