@@ -73,7 +73,9 @@ __device__ __forceinline__ Orbit orbit_setup(const double el_in[6], double gm, d
     // seen by the observer, asin(v_max / c) with v_max the perihelion speed (|r(t) - r(t - tau)| <=
     // v_max tau and tau = rho0 / c exactly, so the bound does not depend on rho0), + slack.
     const double vmax = sqrt(gm / a * (1.0 + e) / (1.0 - e));
-    const double th = atan(tan_fov) * 1.01 + 1.05 * asin(fmin(vmax * inv_c, 1.0)) + 1.4e-4;
+    // The 1e-4 rad of slack for the cull-quality Kepler chain (below) was derived and validated for e <= 0.9 (its
+    // truncation grows like e / (1 - e)); no cone for more eccentric orbits: they are refined everywhere.
+    const double th = (e > 0.9) ? 2.0 : atan(tan_fov) * 1.01 + 1.05 * asin(fmin(vmax * inv_c, 1.0)) + 1.4e-4;
     const double cth = (th < 1.5) ? cos(th) : 0.0;
     o.cos2_cull = (th < 1.5) ? cth * cth : 0.0;
     // The cull may run on an UNPOLISHED order-2 Kepler state, off by <= 6e-6 rad in E (k_propagate), i.e.

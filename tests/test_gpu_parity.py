@@ -487,8 +487,9 @@ def test_pinned_elements_zero_copy_matches_device_path():
     assert res["device"][1][17] == -1 and np.isnan(res["device"][0][17])
 
 
+@pytest.mark.parametrize("e_hi", [0.9, 0.99], ids=["e<=0.9", "e<=0.99"])
 @pytest.mark.parametrize("flags", [0, 2], ids=["warm", "cold"])
-def test_perihelion_stress_all_kepler_paths(flags):
+def test_perihelion_stress_all_kepler_paths(flags, e_hi):
     """Eccentric orbits (e up to 0.9) whose perihelion passages fall inside the exposure span, with
     exposure gaps from minutes to weeks: the warm step at its three orders, the wide step, wide
     sub-steps and the cold solve are all taken (counted), and every sky position / pixel coordinate
@@ -503,7 +504,9 @@ def test_perihelion_stress_all_kepler_paths(flags):
     t = np.concatenate([[0.0], np.cumsum(gaps)])
     G = 8                                                    # guide orbits; families of n / G members
     ga = rng.uniform(0.8, 1.6, G)
-    ge = np.concatenate([rng.uniform(0.88, 0.9, G // 2), rng.uniform(0.6, 0.88, G - G // 2)])
+    # e_hi = 0.99: beyond the range of every config (e <= 0.9) but inside what the ABI accepts (e < 1): such orbits
+    # take no cone pre-cull (orbit_setup) and must still match the oracle through every Kepler path
+    ge = np.concatenate([rng.uniform(e_hi - 0.02, e_hi, G // 2), rng.uniform(0.6 if e_hi <= 0.9 else 0.91, e_hi - 0.02, G - G // 2)])
     period = 2 * np.pi / np.sqrt(ds.GM_SUN / ga ** 3)
     t_peri = rng.uniform(0.2, 0.8, G) * t[-1]                # a perihelion passage inside the span
     guides = np.stack([ga, ge, rng.uniform(0, 0.5, G), rng.uniform(0, 2 * np.pi, G), rng.uniform(0, 2 * np.pi, G),
@@ -526,6 +529,10 @@ def test_perihelion_stress_all_kepler_paths(flags):
         trk.load_image_batch(0, np.ones((N, H, W), np.float32))
         snr, hits = trk.stack(el, 0.0)
         st = trk.stats()
+    # the timed path (pre-cull where the orbit has one) finds exactly the oracle's hits
+    want = (ref["pix"][..., 0] >= 0).sum(1)
+    nfl = ref["flag"].astype(np.int64).sum(1)
+    assert np.array_equal(hits[nfl == 0], want[nfl == 0]) and (np.abs(hits - want) <= nfl).all()
     # a guide is seen in every exposure that tracks it; unit images: SNR = sqrt(hits)
     assert hits[0] >= N // G and abs(snr[0] - math.sqrt(hits[0])) < 1e-12
     near = (np.abs(ref["xy"]) < 1e5).all(-1)
