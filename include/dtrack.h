@@ -51,7 +51,8 @@ enum {
     DT_ERR_OOM = -2,
     DT_ERR_CUDA = -3,
     DT_ERR_NOT_LOADED = -4,
-    DT_ERR_STATE = -5
+    DT_ERR_STATE = -5,
+    DT_ERR_TOO_LARGE = -6      /* a size beyond a fixed capacity (dt_threshold_noalloc)            */
 };
 enum { DT_MEM_HOST = 0, DT_MEM_PINNED = 1, DT_MEM_DEVICE = 2 };
 
@@ -207,6 +208,28 @@ int dt_set_outlier_clip(dt_context *ctx, double clip);
  */
 int dt_threshold(dt_context *ctx, double snr_min, int32_t min_hits, int64_t max_out, int64_t *index_out,
                  double *snr_out, int64_t *n_found);
+
+/*
+ * dt_threshold_noalloc: threshold mode (as dt_threshold: Algorithm 1 `FindSignificantResults`, PAPER.md:173,
+ * 336) for callers that cannot allocate -- code under CUDA graph capture, tight serving loops.  No context:
+ * it works on the CURRENT device, on `stream` (a cudaStream_t passed as a plain pointer; NULL = default
+ * stream), over the caller's DEVICE arrays snr_dev [n] fp64 and hits_dev [n] int32 (e.g. dt_stack's
+ * DT_MEM_DEVICE outputs), and writes DEVICE outputs: *n_found_dev = how many orbits have finite SNR >=
+ * snr_min and hits >= min_hits; index_out_dev [max_out] int64 and snr_out_dev [max_out] fp64 (may be NULL)
+ * get the first min(*n_found_dev, max_out) of them in ascending orbit index (entries beyond that are left
+ * untouched).  The call only enqueues work: no cudaMalloc / cudaFree or allocating library routine, no host
+ * copy, no synchronisation; results are valid once `stream` has reached the end of the call's work, and the
+ * caller owns every array it passes.
+ * Scratch: a static device array of 16.0 MiB built into the library (every GPU that loads the library holds
+ * it until the process exits), sized for n <= DT_NOALLOC_MAX_ORBITS; larger n is DT_ERR_TOO_LARGE (nothing
+ * is enqueued).  All calls on a device share that array: calls must not overlap on the GPU (same stream, or
+ * ordered by events) -- overlapping calls race.  Errors: DT_ERR_INVALID_ARG (NULL arrays, negative sizes, NaN
+ * snr_min), DT_ERR_TOO_LARGE, DT_ERR_CUDA; dt_last_error(NULL) describes the last one.
+ */
+#define DT_NOALLOC_MAX_ORBITS 1048576
+int dt_threshold_noalloc(void *stream, const double *snr_dev, const int32_t *hits_dev, int64_t n, double snr_min,
+                         int32_t min_hits, int64_t max_out, int64_t *index_out_dev, double *snr_out_dev,
+                         int64_t *n_found_dev);
 
 /*
  * Exposure-sharded search.  The paper partitions the IMAGES across ranks without

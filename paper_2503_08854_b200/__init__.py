@@ -25,10 +25,11 @@ DT_OK, DT_ERR_INVALID_ARG, DT_ERR_OOM, DT_ERR_CUDA, DT_ERR_NOT_LOADED, DT_ERR_ST
 DT_MEM_HOST, DT_MEM_PINNED, DT_MEM_DEVICE = 0, 1, 2
 DT_FLAG_FORCE_STREAM, DT_FLAG_KEPLER_COLD, DT_FLAG_NO_PRECULL, DT_FLAG_PROJECT_PRECULL = 1, 2, 4, 8
 _ERR_NAMES = {-1: "DT_ERR_INVALID_ARG", -2: "DT_ERR_OOM", -3: "DT_ERR_CUDA", -4: "DT_ERR_NOT_LOADED",
-              -5: "DT_ERR_STATE"}
+              -5: "DT_ERR_STATE", -6: "DT_ERR_TOO_LARGE"}
+DT_NOALLOC_MAX_ORBITS = 1 << 20
 
 EXPORTS = ["dt_create", "dt_destroy", "dt_load_image_batch", "dt_stack", "dt_stack_epochs", "dt_set_patch",
-           "dt_set_outlier_clip", "dt_threshold", "dt_partials_sparse", "dt_partials_reset", "dt_partials_add",
+           "dt_set_outlier_clip", "dt_threshold", "dt_threshold_noalloc", "dt_partials_sparse", "dt_partials_reset", "dt_partials_add",
            "dt_partials_finalize", "dt_topk", "dt_project",
            "dt_gather_hits", "dt_filter_intersections", "dt_set_option", "dt_get_stats", "dt_last_error", "dt_version", "dt_fp64_peak", "dt_probe_random_gather"]
 
@@ -80,6 +81,7 @@ def lib():
         L.dt_set_patch.argtypes = [vp, C.c_int32, dp]
         L.dt_set_outlier_clip.argtypes = [vp, C.c_double]
         L.dt_threshold.argtypes = [vp, C.c_double, C.c_int32, C.c_int64, C.POINTER(C.c_int64), dp, C.POINTER(C.c_int64)]
+        L.dt_threshold_noalloc.argtypes = [vp, vp, vp, C.c_int64, C.c_double, C.c_int32, C.c_int64, vp, vp, vp]
         L.dt_partials_sparse.argtypes = [vp, C.c_int64, vp, vp, vp, vp, C.c_int32, C.POINTER(C.c_int64)]
         L.dt_partials_reset.argtypes = [vp]
         L.dt_partials_add.argtypes = [vp, vp, vp, vp, vp, C.c_int64, C.c_int32]
@@ -105,7 +107,7 @@ def lib():
 
 def _check(rc: int, ctx=None):
     if rc != DT_OK:
-        msg = lib().dt_last_error(ctx).decode() if ctx else ""
+        msg = lib().dt_last_error(ctx).decode()        # ctx None: the message of the last context-free call
         raise DtError(rc, msg)
 
 
@@ -238,6 +240,22 @@ def dt_threshold(ctx, snr_min: float, min_hits: int = 0, max_out: int = 1 << 20)
                               _dp(val), C.byref(nf)), ctx)
     m = min(nf.value, max_out)
     return idx[:m].copy(), val[:m].copy(), nf.value
+
+
+def dt_threshold_noalloc(snr, hits, snr_min: float, min_hits, index_out, snr_out, n_found, stream=None):
+    """dt_threshold over DEVICE tensors without any allocation (dtrack.h): snr [n] f64, hits [n] i32 in;
+    index_out [max_out] i64, snr_out [max_out] f64 or None, n_found [1] i64 out -- all torch CUDA tensors the
+    caller made, on the current device.  Enqueues on `stream` (a torch.cuda.Stream; default: the current one)
+    and returns without synchronising.  n <= DT_NOALLOC_MAX_ORBITS, else DtError(DT_ERR_TOO_LARGE)."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream(snr.device)
+    assert snr.dtype == torch.float64 and hits.dtype == torch.int32 and index_out.dtype == torch.int64
+    assert n_found.dtype == torch.int64 and (snr_out is None or snr_out.dtype == torch.float64)
+    assert snr.is_contiguous() and hits.is_contiguous() and index_out.is_contiguous() and hits.numel() == snr.numel()
+    max_out = index_out.numel() if snr_out is None else min(index_out.numel(), snr_out.numel())
+    _check(lib().dt_threshold_noalloc(st.cuda_stream, snr.data_ptr(), hits.data_ptr(), snr.numel(), float(snr_min),
+                                      int(min_hits), max_out, index_out.data_ptr(),
+                                      snr_out.data_ptr() if snr_out is not None else None, n_found.data_ptr()))
 
 
 def dt_partials_sparse(ctx, n: int, device=None):

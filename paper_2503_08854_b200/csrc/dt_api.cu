@@ -930,6 +930,31 @@ int dt_threshold(dt_context *c, double snr_min, int32_t min_hits, int64_t max_ou
     return DT_OK;
 }
 
+int dt_threshold_noalloc(void *stream, const double *snr_dev, const int32_t *hits_dev, int64_t n, double snr_min,
+                         int32_t min_hits, int64_t max_out, int64_t *index_out_dev, double *snr_out_dev,
+                         int64_t *n_found_dev)
+{
+    if (n < 0 || max_out < 0 || isnan(snr_min) || !n_found_dev || (n > 0 && (!snr_dev || !hits_dev)) ||
+        (n > 0 && max_out > 0 && !index_out_dev)) {
+        g_static_err = "dt_threshold_noalloc: bad arguments";
+        return DT_ERR_INVALID_ARG;
+    }
+    if (n > threshold_noalloc_max()) {
+        g_static_err = "dt_threshold_noalloc: n exceeds DT_NOALLOC_MAX_ORBITS (1048576), the size the library's static "
+                       "scratch array is built for; split the array or use dt_threshold";
+        return DT_ERR_TOO_LARGE;
+    }
+    static_assert(sizeof(long long) == sizeof(int64_t), "int64");
+    const cudaError_t e = threshold_noalloc_device(snr_dev, hits_dev, n, snr_min, min_hits, max_out,
+                                                   reinterpret_cast<long long *>(index_out_dev), snr_out_dev,
+                                                   reinterpret_cast<long long *>(n_found_dev), (cudaStream_t)stream);
+    if (e != cudaSuccess) {
+        g_static_err = cudaGetErrorString(e);
+        return DT_ERR_CUDA;
+    }
+    return DT_OK;
+}
+
 static int partial_scratch(dt_context *c, int64_t m)
 {
     if (m <= c->p_cap && c->d_pidx) return DT_OK;

@@ -143,6 +143,13 @@ cudaError_t threshold_device(const double *snr, const int32_t *hits, int64_t n, 
                              int32_t min_hits, int64_t max_out, TopkWorkspace &ws, int64_t *index_out_host,
                              double *snr_out_host, int64_t *n_found, cudaStream_t stream);
 
+// The same without any allocation, host copy or synchronisation: scratch in a file-scope device array of dt_topk.cu,
+// inputs and outputs DEVICE arrays (dtrack.h dt_threshold_noalloc); n <= threshold_noalloc_max().
+cudaError_t threshold_noalloc_device(const double *snr, const int32_t *hits, int64_t n, double snr_min,
+                                     int32_t min_hits, int64_t max_out, long long *index_out_dev,
+                                     double *snr_out_dev, long long *n_found_dev, cudaStream_t stream);
+int64_t threshold_noalloc_max();
+
 // FP64 FMA issue-rate probe (dt_fp64_peak).
 cudaError_t fp64_peak_device(double *tflops, cudaStream_t stream);
 // Random 4-B gather rate over a buffer of buffer_bytes (dt_probe_random_gather).

@@ -562,6 +562,97 @@ cudaError_t refinalize_device(int64_t n, const double *S, const double *Wt, cons
     return cudaGetLastError();
 }
 
+// ---- threshold mode without any allocation (dtrack.h dt_threshold_noalloc) -------------------------------------
+// For callers that must not call cudaMalloc (CUDA graph capture, tight serving loops): the same ordered
+// compaction as threshold_device -- same kernels, same order -- over the caller's DEVICE arrays, with every
+// intermediate in ONE file-scope device array and every result written to the caller's DEVICE arrays, so the
+// call enqueues kernels (and one 8-byte device-to-device copy) and nothing else: no allocation, no host copy, no
+// synchronisation.  The array is part of the library image: every GPU that loads the library holds its
+// kNoAllocBytes until the process exits.  Its name is a HOST-side stand-in in host code: the address the kernels
+// get is the one cudaGetSymbolAddress returns, taken once per device with that device current.  All calls on a
+// device share the array, and it keeps the last call's contents: the state words are cleared by every call, the
+// key / candidate / block-count regions are fully rewritten before they are read.  Two calls that overlap on
+// the GPU (different streams, no ordering between them) race on it.
+constexpr int64_t kNoAllocMaxOrbits = 1 << 20;                                         // DT_NOALLOC_MAX_ORBITS
+constexpr int64_t kNoAllocBlocks = (kNoAllocMaxOrbits + kChunk - 1) / kChunk;
+constexpr size_t kNoAllocKeys = 0;                                                     // [max] u64 keys
+constexpr size_t kNoAllocCand = kNoAllocKeys + (size_t)kNoAllocMaxOrbits * 8;          // [max] u64 candidate keys
+constexpr size_t kNoAllocCounts = kNoAllocCand + (size_t)kNoAllocMaxOrbits * 8;        // [2 blocks] u32
+constexpr size_t kNoAllocState = kNoAllocCounts + ((size_t)kNoAllocBlocks * 8 + 255) / 256 * 256;   // [16] u64
+constexpr size_t kNoAllocBytes = kNoAllocState + 256;                                  // 16.0 MiB + 2.25 KiB
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+namespace {
+
+// the first min(total, max_out) candidates' SNR, `total` read on the device (state[7], written by k_scan)
+__global__ void k_emit_counted(const long long *__restrict__ cand_idx, const double *__restrict__ snr,
+                               const unsigned long long *__restrict__ state, int64_t max_out,
+                               double *__restrict__ out_snr)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t m = min((int64_t)state[7], max_out);
+    if (i < m) out_snr[i] = snr[cand_idx[i]];
+}
+
+constexpr int kNoAllocMaxDevices = 64;
+unsigned char *g_noalloc_addr[kNoAllocMaxDevices];      // device address of g_noalloc_scratch, per device ordinal
+
+}  // namespace
+
+int64_t threshold_noalloc_max() { return kNoAllocMaxOrbits; }
+
+// The current device's address of the scratch array (set-up: once per device, that device current).
+static cudaError_t noalloc_scratch_address(unsigned char **out)
+{
+    int dev = -1;
+    TK_CHECK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return cudaErrorInvalidDevice;
+    unsigned char *p = __atomic_load_n(&g_noalloc_addr[dev], __ATOMIC_ACQUIRE);
+    if (!p) {
+        void *sym = nullptr;
+        TK_CHECK(cudaGetSymbolAddress(&sym, g_noalloc_scratch));     // the host-side name is NOT this address
+        if (!sym) return cudaErrorInvalidSymbol;
+        p = static_cast<unsigned char *>(sym);
+        __atomic_store_n(&g_noalloc_addr[dev], p, __ATOMIC_RELEASE);   // racing threads store the same value
+    }
+    *out = p;
+    return cudaSuccess;
+}
+
+cudaError_t threshold_noalloc_device(const double *snr, const int32_t *hits, int64_t n, double snr_min,
+                                     int32_t min_hits, int64_t max_out, long long *index_out_dev,
+                                     double *snr_out_dev, long long *n_found_dev, cudaStream_t stream)
+{
+    if (n < 0 || n > kNoAllocMaxOrbits) return cudaErrorInvalidValue;      // the caller reports the limit
+    unsigned char *base = nullptr;
+    TK_CHECK(noalloc_scratch_address(&base));
+    unsigned long long *keys = reinterpret_cast<unsigned long long *>(base + kNoAllocKeys);
+    unsigned long long *cand_key = reinterpret_cast<unsigned long long *>(base + kNoAllocCand);
+    unsigned int *counts = reinterpret_cast<unsigned int *>(base + kNoAllocCounts);
+    unsigned long long *state = reinterpret_cast<unsigned long long *>(base + kNoAllocState);
+    TK_CHECK(cudaMemsetAsync(state, 0, 16 * sizeof(unsigned long long), stream));   // also the count of an empty call
+    if (n > 0) {
+        const int nblocks = (int)((n + kChunk - 1) / kChunk);
+        double th = (snr_min == 0.0) ? -0.0 : snr_min;                     // as threshold_device
+        unsigned long long b;
+        memcpy(&b, &th, sizeof b);
+        const unsigned long long key = (b & 0x8000000000000000ull) ? ~b : (b | 0x8000000000000000ull);
+        k_keys<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(snr, hits, n, min_hits, keys);
+        k_set_threshold<<<1, 1, 0, stream>>>(state, key - 1ull);
+        k_count<<<nblocks, kThreads, 0, stream>>>(keys, n, state, counts);
+        k_scan<<<1, 1024, 0, stream>>>(counts, nblocks, state);
+        // at most min(max_out, n) <= kNoAllocMaxOrbits candidates are written
+        k_scatter<<<nblocks, kThreads, 0, stream>>>(keys, n, state, counts, cand_key, index_out_dev,
+                                                    (unsigned long long)max_out);
+        const int64_t cap = std::min<int64_t>(max_out, n);
+        if (snr_out_dev && cap > 0)
+            k_emit_counted<<<(unsigned)((cap + 255) / 256), 256, 0, stream>>>(index_out_dev, snr, state, max_out,
+                                                                             snr_out_dev);
+        TK_CHECK(cudaGetLastError());
+    }
+    return cudaMemcpyAsync(n_found_dev, state + 7, sizeof(long long), cudaMemcpyDeviceToDevice, stream);
+}
+
 void topk_free(TopkWorkspace &ws)
 {
     cudaFree(ws.keys);
