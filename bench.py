@@ -450,6 +450,7 @@ def gather_bench(dt, trk, cfg, dev, hbm_gbs, flush, reps=5, regimes=None):
     n = min(cfg.n_orbits, 1 << 20)
     G = max(1, min(cfg.n_exp // 32, 15))
     out = []
+    l2_rate = None
     words = 2 if cfg.variance_mode == 1 else 1
     for name, cluster, density in (regimes or GATHER_REGIMES):
         hl = hitlists.build(n, G, cfg.width, cfg.height, cluster, density, 7, dev, px_per_sector=8 // words)
@@ -472,14 +473,21 @@ def gather_bench(dt, trk, cfg, dev, hbm_gbs, flush, reps=5, regimes=None):
         bytes_min = (hl["hits"] * 4 + hl["mask"].numel() * 4 + hl["base"].numel() * 8 +
                      hl["unique_sectors"] * 32 + hl["touched_orbits"] * 20)
         gbs = bytes_min / (ms * 1e-3) * 1e-9
-        # second bound: a fully divergent 4-B gather is served by the L1 at one lane per clock and SM
+        # second bound: a fully divergent 4-B gather is served by the L1 at one lane per clock and SM at best;
+        # third: the rate the part really gives fully divergent gathers that HIT the L2 (measured by the probe over
+        # one 16 MiB plane-sized buffer): the dense schedule keeps the planes L2-resident, so this is its ceiling
         props = torch.cuda.get_device_properties(dev)
         l1_rate = props.multi_processor_count * sm_clock_hz(dev.index or 0)
+        if l2_rate is None:
+            l2_rate = dt.dt_probe_random_gather(dev.index or 0, 16 << 20, 0)
         out.append({"regime": name, "image_set": cfg.name, "hits": hl["hits"], "unique_sectors": hl["unique_sectors"],
                     "bytes_min": int(bytes_min), "ms": ms, "hits_per_s": hl["hits"] / (ms * 1e-3),
                     "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": gbs / hbm_gbs,
                     "l1_gather_bound": {"peak": l1_rate, "unit": "gathers/s",
-                                        "frac": hl["hits"] / (ms * 1e-3) / l1_rate}})
+                                        "frac": hl["hits"] / (ms * 1e-3) / l1_rate},
+                    "l2_gather_bound": {"peak": l2_rate, "unit": "gathers/s",
+                                        "peak_source": "dt_probe_random_gather over a 16 MiB (L2-resident) buffer, this run",
+                                        "frac": hl["hits"] / (ms * 1e-3) / l2_rate}})
         del hl, S, Wt, cnt
         torch.cuda.empty_cache()
     return out
@@ -577,6 +585,7 @@ def run_config(dt, args, name, dev, local_rank, rank, world, steps, warmup, flus
                  "stages_ms": {"propagate": ms_prop, "gather": ms_gath, "finalize": stats["ms_finalize"]},
                  "hits_per_step": int(stats["hits"]), "refined_pairs": int(stats["refined_pairs"]),
                  "cold_solves": int(stats["cold_solves"]), "substep_solves": int(stats["substep_solves"]),
+                 "gated_pairs": int(stats["gated_pairs"]),
                  "launches_per_step": int(stats["launches"]),
                  "images_resident": not bool(stats["streamed"]), "image_zero_copy": bool(stats["image_zero_copy"]),
                  "h2d_image_bytes_per_step": int(stats["h2d_image_bytes"]), "build_s": t_build,
@@ -647,7 +656,11 @@ def main():
         out = {}
         for hint in (0, 1):
             out["ld.global.nc" + (".L2::64B" if hint else "")] = dt.dt_probe_random_gather(local_rank, 8 << 30, hint)
-        print(json.dumps({"probe_random_gather": {"unit": "4-B gathers/s over an 8 GiB buffer", **out}}))
+        res = dt.dt_probe_random_gather(local_rank, 16 << 20, 0)
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        print(json.dumps({"probe_random_gather": {"unit": "4-B gathers/s over an 8 GiB buffer", **out,
+                                                  "l2_resident_16MiB": res,
+                                                  "l2_resident_lanes_per_clock_and_sm": res / (sms * sm_clock_hz(local_rank))}}))
         return
 
     if args.count_k1:
@@ -668,12 +681,21 @@ def main():
         el = elements_device(cfg, 0, cfg.n_orbits, dev)
         st = {"pairs": 0, "hits": 0, "propagate_launches": 0}
         with dt.Tracker.from_scene(scene, device=local_rank, flags=args.flags) as trk:      # kernel 1 needs no images
-            for first in range(0, cfg.n_exp, UNIT_EXPOSURES):
-                ne = min(UNIT_EXPOSURES, cfg.n_exp - first)
-                hl = trk.filter_intersections(el, scene.t0, first, ne)
-                st["pairs"] += cfg.n_orbits * ne
-                st["hits"] += hl["n_hits"]
-                st["propagate_launches"] += 1
+            # pass 0, unprofiled (the ncu command says --profile-from-start off): the device-side choice of the
+            # kernel-1 variant settles, as it has for all but the first of a full step's ~100 units; pass 1 is counted
+            for counted in (False, True):
+                if counted:
+                    torch.cuda.synchronize()
+                    torch.cuda.cudart().cudaProfilerStart()
+                for first in range(0, cfg.n_exp, UNIT_EXPOSURES):
+                    ne = min(UNIT_EXPOSURES, cfg.n_exp - first)
+                    hl = trk.filter_intersections(el, scene.t0, first, ne)
+                    if counted:
+                        st["pairs"] += cfg.n_orbits * ne
+                        st["hits"] += hl["n_hits"]
+                        st["propagate_launches"] += 1
+            torch.cuda.synchronize()
+            torch.cuda.cudart().cudaProfilerStop()
         os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
         line = "COUNT_K1 workload=%s pairs=%d flags=%d launches=%d hits=%d" % (
             name, st["pairs"], args.flags, st["propagate_launches"], st["hits"])
@@ -770,6 +792,7 @@ def main():
                 "roofline": k1, "step_roofline": entry.get("roofline"),
                 "stages_ms": entry["stages_ms"], "hits_per_step": entry["hits_per_step"],
                 "cold_solves": entry["cold_solves"], "substep_solves": entry["substep_solves"],
+                "gated_pairs": entry["gated_pairs"],
                 "topk_ms": topk_ms, "peaks": peaks, "wall_s_timed_region": wall}
 
     # ---- every BASELINE.json config, literal and focused, at full size ----

@@ -63,10 +63,14 @@ enum {
                                 /* (reference mode of kernel 1; default is the warm-started solve) */
     DT_FLAG_NO_PRECULL = 4,     /* do the light-time refinement + projection for every pair, even  */
                                 /* when a conservative cone test already proves a miss             */
-    DT_FLAG_PROJECT_PRECULL = 8 /* dt_project runs kernel 1 exactly as dt_stack does, pre-cull and */
+    DT_FLAG_PROJECT_PRECULL = 8, /* dt_project runs kernel 1 exactly as dt_stack does, pre-cull and */
                                 /* cull-quality Kepler chain included: a pair the cone test rejects */
                                 /* is reported as culled (NaN, (-1,-1)).  For parity tests of the   */
                                 /* path the timed kernel takes; default dt_project refines all.    */
+    DT_FLAG_NO_GROUP_GATE = 16  /* never use the group ephemeris gate (one Kepler solve per orbit   */
+                                /* and group of 32 exposures + a second-order Taylor position with  */
+                                /* a rigorous remainder bound decide which pairs reach the per-pair */
+                                /* Kepler step; results are identical with and without it)          */
 };
 
 /*
@@ -119,6 +123,7 @@ typedef struct {
     int32_t image_tiles;       /* 1 when a streamed survey went through the tiled image cache: only the   */
                                /* 64 x 64-pixel tiles the hits fall on were copied (h2d_image_bytes)       */
     int64_t tiles_fetched;     /* tiles copied host -> device by the call                                 */
+    int64_t gated_pairs;       /* pairs the group ephemeris gate removed before any per-pair Kepler step  */
 } dt_stats;
 
 /*
@@ -313,6 +318,10 @@ int dt_filter_intersections(dt_context *ctx, const double *elements, int64_t n, 
 
 /*
  * dt_set_option: tuning knobs of a context (none changes any result; defaults are the measured best).
+ *   "group_gate"          -1 (default): for every work unit the device picks the kernel-1 variant with or without
+ *                         the group ephemeris gate from what the previous unit did (on where warps cull -- a
+ *                         blind search -- and the gate really gates; off where most pairs are refined or the
+ *                         remainder bounds are loose); 0 never, 1 always
  *   "gather_schedule"     -1 chosen on the device from the hit density (default), 0 orbit-major walk,
  *                         1 dense lock-step (one exposure at a time)
  *   "gather_window"       dense schedule: exposures the fastest CTA may be ahead (0 = from the L2 size)
@@ -345,7 +354,10 @@ int dt_fp64_peak(int32_t device, double *tflops);
  * dt_probe_random_gather: what the device gives a gather-bound kernel -- independent 4-B loads at hashed
  * addresses of a buffer of buffer_bytes (rounded down to a power of two; >= 1 MiB), eight in flight per thread;
  * hint64 != 0: the loads carry .L2::64B (a miss fetches 64 B of DRAM instead of 128 B).  Writes gathers per
- * second.  The second roofline denominator of kernel 3 on sparse hit lists.
+ * second.  Over a buffer far beyond the L2 (8 GiB): the random-DRAM-access rate, the second roofline denominator
+ * of kernel 3 on sparse hit lists; over a buffer that stays L2-resident (16 MiB, one 2048^2 plane): the rate of
+ * fully divergent L2-hit gathers through the L1 miss path, the denominator of the dense schedule (DESIGN.md
+ * "Measurement").
  */
 int dt_probe_random_gather(int32_t device, int64_t buffer_bytes, int32_t hint64, double *gathers_per_s);
 

@@ -23,7 +23,7 @@ from . import _build
 
 DT_OK, DT_ERR_INVALID_ARG, DT_ERR_OOM, DT_ERR_CUDA, DT_ERR_NOT_LOADED, DT_ERR_STATE = 0, -1, -2, -3, -4, -5
 DT_MEM_HOST, DT_MEM_PINNED, DT_MEM_DEVICE = 0, 1, 2
-DT_FLAG_FORCE_STREAM, DT_FLAG_KEPLER_COLD, DT_FLAG_NO_PRECULL, DT_FLAG_PROJECT_PRECULL = 1, 2, 4, 8
+DT_FLAG_FORCE_STREAM, DT_FLAG_KEPLER_COLD, DT_FLAG_NO_PRECULL, DT_FLAG_PROJECT_PRECULL, DT_FLAG_NO_GROUP_GATE = 1, 2, 4, 8, 16
 _ERR_NAMES = {-1: "DT_ERR_INVALID_ARG", -2: "DT_ERR_OOM", -3: "DT_ERR_CUDA", -4: "DT_ERR_NOT_LOADED",
               -5: "DT_ERR_STATE", -6: "DT_ERR_TOO_LARGE"}
 DT_NOALLOC_MAX_ORBITS = 1 << 20
@@ -58,7 +58,7 @@ class dt_stats(C.Structure):
                 ("ms_total", C.c_float), ("ms_propagate", C.c_float), ("ms_gather", C.c_float),
                 ("ms_finalize", C.c_float), ("launches", C.c_int32), ("propagate_launches", C.c_int32),
                 ("gather_launches", C.c_int32), ("image_zero_copy", C.c_int32), ("image_tiles", C.c_int32),
-                ("tiles_fetched", C.c_int64)]
+                ("tiles_fetched", C.c_int64), ("gated_pairs", C.c_int64)]
 
 
 _lib = None

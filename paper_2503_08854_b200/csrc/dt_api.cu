@@ -74,6 +74,8 @@ struct dt_context {
     uint32_t *d_offsets = nullptr;
     int64_t mask_cap = 0, base_cap = 0, off_cap = 0;
     unsigned long long *d_counters = nullptr;           // [8]
+    GatePolicy *d_policy = nullptr;                     // kernel-1 variant of the next unit (device-side choice)
+    int32_t group_gate = -1;                            // -1 chosen on the device, 0 never, 1 always
     int *d_progress = nullptr;                          // kernel 3 lock-step counters, one per exposure of a unit
     int32_t gather_window = 1;                          // exposures the slowest and fastest CTA may be apart
     int32_t gather_lockstep = -1;                       // schedule: -1 decided on the device from the hit density
@@ -171,6 +173,7 @@ void free_all(dt_context *c)
     cudaFree(c->d_base);
     cudaFree(c->d_offsets);
     cudaFree(c->d_counters);
+    cudaFree(c->d_policy);
     cudaFree(c->d_progress);
     cudaFree(c->tile_count);
     cudaFree(c->tile_slot);
@@ -367,6 +370,11 @@ int dt_create(const dt_survey *s, dt_context **out)
         if (cudaMemcpyAsync(c->d_exp, c->h_exp.data(), sizeof(ExpRec) * (size_t)c->N, cudaMemcpyHostToDevice,
                             c->stream) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
         if (cudaMalloc((void **)&c->d_counters, 8 * sizeof(unsigned long long)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
+        if (cudaMalloc((void **)&c->d_policy, sizeof(GatePolicy)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
+        {
+            const GatePolicy first = {1, 0, 0ull, 0ull};          // a context starts with the gate on
+            if (cudaMemcpy(c->d_policy, &first, sizeof first, cudaMemcpyHostToDevice) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
+        }
         if (cudaMalloc((void **)&c->d_progress, (size_t)(kMaxUnitExposures + kGroup) * kProgressStride * sizeof(int)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
         c->gather_window = pick_gather_window(c);
         // kernel attributes are per DEVICE: set them for this context's device (no process-wide statics)
@@ -468,6 +476,34 @@ static int propagate_mode(const dt_context *c)
     if (!(c->flags & DT_FLAG_KEPLER_COLD)) mode |= kModeWarm;
     if (!(c->flags & DT_FLAG_NO_PRECULL)) mode |= kModePrecull;
     return mode;
+}
+
+// the call's counters restart from zero, and with them the policy's snapshots of two of them (its choice is kept)
+static cudaError_t reset_counters(dt_context *c)
+{
+    cudaError_t e = cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream);
+    if (e != cudaSuccess) return e;
+    return cudaMemsetAsync(&c->d_policy->refined0, 0, 2 * sizeof(unsigned long long), c->stream);
+}
+
+// Kernel 1 of one unit.  The group ephemeris gate (dt_orbit.cuh) exists for the default mode only (warm chain +
+// pre-cull); unless an option or a flag fixes it, BOTH variants are enqueued -- the one the device-side policy does
+// not name returns at once -- and the policy is updated from what the unit did: no host synchronisation.
+static cudaError_t launch_k1_unit(dt_context *c, PropagateParams &p, int mode, int32_t *launches)
+{
+    const bool can_gate = mode == (kModeWarm | kModePrecull);
+    const int gate = (!can_gate || (c->flags & DT_FLAG_NO_GROUP_GATE)) ? 0 : c->group_gate;
+    p.policy = nullptr;
+    if (gate >= 0) {
+        *launches += 1;
+        return launch_propagate(p, gate ? (mode | kModeGate) : mode, c->stream);
+    }
+    p.policy = c->d_policy;
+    cudaError_t e = launch_propagate(p, mode | kModeGate, c->stream);
+    if (e == cudaSuccess) e = launch_propagate(p, mode, c->stream);
+    if (e == cudaSuccess) e = launch_gate_policy(c->d_policy, c->d_counters, p.n_orbits * (int64_t)p.n_exp, c->stream);
+    *launches += 3;
+    return e;
 }
 
 static void fill_gather_ext(const dt_context *c, GatherParams &g)
@@ -598,9 +634,10 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
     CU(c, cudaMemsetAsync(c->d_S, 0, (size_t)n * 8, c->stream));
     CU(c, cudaMemsetAsync(c->d_Wt, 0, (size_t)n * 8, c->stream));
     CU(c, cudaMemsetAsync(c->d_cnt, 0, (size_t)n * 4, c->stream));
-    CU(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+    CU(c, reset_counters(c));
 
     const int mode = propagate_mode(c);
+    int32_t k1_launches = 0;        // kernels enqueued for kernel 1: one per unit, or both variants + the policy update
 
     auto issue_copy = [&](int b) -> int {
         const int slot = b & 1;
@@ -668,12 +705,12 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
                 p.base = c->d_base;
                 p.offsets = c->d_offsets;
                 p.counters = c->d_counters;
-                CU(c, launch_propagate(p, mode, c->stream));
+                CU(c, launch_k1_unit(c, p, mode, &k1_launches));
                 st.propagate_launches += 1;
                 unsigned long long probe_hits = 0;
                 CU(c, cudaMemcpyAsync(&probe_hits, c->d_counters, sizeof probe_hits, cudaMemcpyDeviceToHost, c->stream));
                 CU(c, cudaStreamSynchronize(c->stream));
-                CU(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+                CU(c, reset_counters(c));
                 const double planes = (c->var_mode == 1) ? 2.0 : 1.0;
                 const double gathers = (double)probe_hits / ((double)no * ne) * (double)n * c->N * planes;
                 zero_copy_images = gathers * 128.0 < 0.05 * (double)c->N * (double)c->plane * 4.0 * planes;
@@ -750,7 +787,7 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
             // the hit counter restarts per unit so offsets index from 0
             CU(c, cudaMemsetAsync(c->d_counters, 0, sizeof(unsigned long long), c->stream));
             CU(c, cudaEventRecord(ev_at(3 * unit_idx), c->stream));
-            CU(c, launch_propagate(p, mode, c->stream));
+            CU(c, launch_k1_unit(c, p, mode, &k1_launches));
             st.propagate_launches += 1;
             CU(c, cudaEventRecord(ev_at(3 * unit_idx + 1), c->stream));
 
@@ -867,9 +904,10 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
     st.cold_solves = (int64_t)hc[2];
     st.substep_solves = (int64_t)hc[4];
     st.invalid_orbits = (int64_t)hc[5];
+    st.gated_pairs = (int64_t)hc[6];
     if (hc[7] != 0)
         return fail(c, DT_ERR_CUDA, "bounds-check build: %llu out-of-bounds indices were caught on the device", hc[7]);
-    st.launches = st.propagate_launches + st.gather_launches + 1;
+    st.launches = k1_launches + st.gather_launches + 1;
     c->n_last = n;
     return DT_OK;
 }
@@ -1098,9 +1136,11 @@ int dt_project(dt_context *c, const double *elements, int64_t n, double t0, doub
     CUP(cudaMalloc((void **)&d_radec, (size_t)chunk * N * 16));
     CUP(cudaMalloc((void **)&d_xy, (size_t)chunk * N * 16));
     CUP(cudaMalloc((void **)&d_pix, (size_t)chunk * N * 8));
-    // default: every pair refined; DT_FLAG_PROJECT_PRECULL keeps dt_stack's pre-cull and cull-quality chain
-    const int mode = (propagate_mode(c) & (kModeWarm | ((c->flags & DT_FLAG_PROJECT_PRECULL) ? kModePrecull : 0))) |
-                     kModeDense;
+    // default: every pair refined; DT_FLAG_PROJECT_PRECULL keeps dt_stack's pre-cull and cull-quality chain, and the
+    // group ephemeris gate unless it is switched off (no device-side choice here: a parity entry runs what it is told)
+    int mode = propagate_mode(c) & (kModeWarm | ((c->flags & DT_FLAG_PROJECT_PRECULL) ? kModePrecull : 0));
+    if (mode == (kModeWarm | kModePrecull) && !(c->flags & DT_FLAG_NO_GROUP_GATE) && c->group_gate != 0) mode |= kModeGate;
+    mode |= kModeDense;
     for (int64_t o0 = 0; o0 < n; o0 += chunk) {
         const int64_t no = std::min<int64_t>(chunk, n - o0);
         CUP(cudaMemcpyAsync(d_el, elements + o0 * 6, (size_t)no * 48, cudaMemcpyHostToDevice, c->stream));
@@ -1207,7 +1247,7 @@ int dt_filter_intersections(dt_context *c, const double *elements, int64_t n, do
     CU(c, grow(c->d_mask, c->mask_cap, pad * groups));
     CU(c, grow(c->d_base, c->base_cap, (pad / 32) * groups));
     CU(c, grow(c->d_offsets, c->off_cap, pad * (int64_t)groups * kGroup));
-    CU(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+    CU(c, reset_counters(c));
     PropagateParams p;
     fill_common(c, p, t0);
     p.elements = d_el;
@@ -1220,7 +1260,8 @@ int dt_filter_intersections(dt_context *c, const double *elements, int64_t n, do
     p.base = c->d_base;
     p.offsets = c->d_offsets;
     p.counters = c->d_counters;
-    CU(c, launch_propagate(p, propagate_mode(c), c->stream));
+    int32_t k1_launches = 0;
+    CU(c, launch_k1_unit(c, p, propagate_mode(c), &k1_launches));
     unsigned long long h = 0;
     CU(c, cudaMemcpyAsync(&h, c->d_counters, sizeof h, cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
@@ -1241,6 +1282,9 @@ int dt_set_option(dt_context *c, const char *name, int64_t value)
     if (k == "gather_schedule") {
         if (value < -1 || value > 1) return fail(c, DT_ERR_INVALID_ARG, "gather_schedule: -1 auto, 0 orbit-major, 1 dense");
         c->gather_lockstep = (int32_t)value;
+    } else if (k == "group_gate") {
+        if (value < -1 || value > 1) return fail(c, DT_ERR_INVALID_ARG, "group_gate: -1 chosen on the device, 0 off, 1 on");
+        c->group_gate = (int32_t)value;
     } else if (k == "gather_window") {
         c->gather_window = value > 0 ? (int32_t)std::min<int64_t>(value, 64) : pick_gather_window(c);
     } else if (k == "gather_prefetch") {

@@ -43,6 +43,7 @@ constexpr int kTileOrbits = DT_K1_TILE;   // orbits per CTA of kernel 1 (one orb
 constexpr int kWarpsPerCta = kTileOrbits / 32;
 
 // ---- kernel 1 (+2): propagate, project, cull, compact ------------------------------------------
+struct GatePolicy;
 struct PropagateParams {
     const double *elements;     // [n][6], 16-B aligned; device memory or device-mapped pinned host memory
     double *elements_copy;      // NULL, or device [n][6]: the kernel leaves a copy of what it read
@@ -62,13 +63,25 @@ struct PropagateParams {
     unsigned long long *base;   // [n_groups][n_pad/32]
     uint32_t *offsets;          // [capacity]
     int64_t offsets_cap;        // entries `offsets` can hold (bounds-check build)
-    unsigned long long *counters;  // [0] unit hit allocator, [1] refined pairs, [2] cold solves, [3] hits, [7] bounds violations
+    unsigned long long *counters;  // [0] unit hit allocator, [1] refined pairs, [2] cold solves, [3] hits, [4] sub-step solves, [6] gated pairs, [7] bounds violations
+    const GatePolicy *policy;   // NULL, or: the kernel returns at once unless policy->select says its variant runs
     // dense debug outputs (dt_project), NULL on the timed path
     double *radec, *xy;         // [n][n_exp][2]
     int32_t *pix;               // [n][n_exp][2]
 };
 
-enum { kModeWarm = 1, kModePrecull = 2, kModeDense = 4 };
+enum { kModeWarm = 1, kModePrecull = 2, kModeDense = 4, kModeGate = 8 };   // kModeGate: with kModeWarm | kModePrecull only
+
+// Device-side choice between the kernel-1 variants with and without the group ephemeris gate (dt_orbit.cuh): both are
+// enqueued for every unit and the one `select[0]` does not name returns at once, so the choice needs no host
+// synchronisation.  k_gate_policy (dt_propagate.cu) sets it after every unit from what that unit did.
+struct GatePolicy {
+    int32_t select;                 // 1: the next unit runs the gate variant
+    int32_t cooldown;               // units left before a gate that proved useless is tried again
+    unsigned long long refined0, gated0;   // counters[1], counters[6] at the end of the previous unit
+};
+cudaError_t launch_gate_policy(GatePolicy *policy, const unsigned long long *counters, int64_t unit_pairs,
+                               cudaStream_t stream);
 
 cudaError_t launch_propagate(const PropagateParams &p, int mode, cudaStream_t stream);
 

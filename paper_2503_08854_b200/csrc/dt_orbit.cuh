@@ -30,6 +30,7 @@ struct Orbit {
     double Ax, Ay, Az, Bx, By, Bz;  // equatorial, AU
     double cos2_cull;               // cos^2 of the pre-cull cone half-angle
     double rho2_close;              // pairs closer than this (AU^2) are always refined
+    double vmax;                    // perihelion speed, AU / day (the largest speed on the orbit)
     bool valid;
 };
 
@@ -73,6 +74,7 @@ __device__ __forceinline__ Orbit orbit_setup(const double el_in[6], double gm, d
     // seen by the observer, asin(v_max / c) with v_max the perihelion speed (|r(t) - r(t - tau)| <=
     // v_max tau and tau = rho0 / c exactly, so the bound does not depend on rho0), + slack.
     const double vmax = sqrt(gm / a * (1.0 + e) / (1.0 - e));
+    o.vmax = vmax;
     // The 1e-4 rad of slack for the cull-quality Kepler chain (below) was derived and validated for e <= 0.9 (its
     // truncation grows like e / (1 - e)); no cone for more eccentric orbits: they are refined everywhere.
     const double th = (e > 0.9) ? 2.0 : atan(tan_fov) * 1.01 + 1.05 * asin(fmin(vmax * inv_c, 1.0)) + 1.4e-4;
@@ -483,6 +485,89 @@ __device__ __forceinline__ Kepler kepler_refresh(double e, const Kepler &K0)
     K.s = fma(d, c, s);
     K.c = fma(-d, s, c);
     return K;
+}
+
+// ---- group ephemeris gate (reading A25) ------------------------------------------------------------
+// A blind search culls all but ~1e-6 of its pairs, and the cull above still pays a Kepler step per pair.  The gate
+// replaces that step, for one exposure group at a time, by the second-order Taylor expansion of the heliocentric
+// position about the group's mid-time tm,
+//     T2(tau) = r + v tau + (a/2) tau^2,   v = (dE/dt)(-A sin E + B cos E),  dE/dt = n / (1 - e cos E),
+//                                           a = -(GM / |r|^3) r = -n^2 (1 - e cos E)^-3 r,
+// from ONE polished Kepler solve per (orbit, group), and culls a pair when T2 - R_obs lies outside a cone that is
+// widened by everything T2 leaves out -- rigorously, so that no pair the exact path would report can be lost:
+//   * Taylor remainder: |r(t) - T2| <= |tau|^3 / 6 sup |d3r/dt3|, and d3r/dt3 = -GM (v / r^3 - 3 (r.v) r / r^5)
+//     gives |d3r/dt3| <= 4 GM |v| / r^3; over the group r >= rmin (below) and |v| <= min(vmax, sqrt(2 GM / rmin))
+//     (vmax: perihelion speed), tau_max the group's half-span;
+//   * light-time: |r(t - lt) - r(t)| <= vmax lt, lt = rho / c, rho <= D / cos(theta_c) <= D (1 + tan theta_c);
+//   * footprint: a hit has D = q.t > 0 and a distance from the pointing axis d_perp <= D tan(theta_c), theta_c the
+//     footprint's half-diagonal (tan_fov, exact for the gnomonic projection).
+// With |delta| <= eps_tot the displacement between the true topocentric vector and T2 - R_obs, D0 and d0 the
+// approximate vector's axial and perpendicular components: D0 >= D - eps_tot and d0 <= (D0 + eps_tot) tan(theta_c)
+// + eps_tot, eps_tot <= (epsT + kappa D0)(1 + 2 kappa), kappa = vmax / (c cos theta_c).  The gate therefore keeps a
+// pair unless D0 < -eps or d0 > D0 tq + eps, with tq and eps below (5 % margins on every term; comparisons are
+// written so that a NaN keeps the pair).  Nothing else changes: a pair the gate keeps goes through the cull-quality
+// chain and the exact cone test as before, from a Kepler state that is at most half a group old.
+struct GroupEph {
+    double tm;                                      // expansion time, days
+    double rx, ry, rz, vx, vy, vz, hx, hy, hz;      // r, v, a / 2 at tm: heliocentric equatorial, AU and days
+    double tq, eps;                                 // keep unless D0 < -eps or d0 > D0 tq + eps
+};
+
+// The gate's two constants.  rmin: a lower bound of |r| over the group.  MUFU seeds + one Newton / Goldschmidt step
+// (1e-12 relative) are plenty under 5 % margins.
+__device__ __forceinline__ double gate_eps_bound(double gm, double vmax, double rmin, double tau_max, double tan_fov)
+{
+    const double rinv = rcp_nr<1>(rmin);
+    const double vint = fmin(vmax, sqrt_nr<1>(2.0 * gm * rinv));
+    const double epsT = 1.05 * (4.0 * gm * vint * (rinv * rinv * rinv)) * (tau_max * tau_max * tau_max) * (1.0 / 6.0);
+    return fma(1.05 * epsT, 1.0 + tan_fov, 1e-12);
+}
+__device__ __forceinline__ double gate_tq(double vmax, double inv_c, double tan_fov)
+{
+    const double kap = 1.05 * vmax * inv_c * (1.0 + tan_fov);   // >= vmax / (c cos theta_c), and its (1 + 2 kappa)
+    // a light-time cone that is no cone (kappa >~ 0.01 needs e -> 1): infinite, the gate then keeps every pair
+    return (kap < 0.01) ? fma(kap, 1.0 + tan_fov, 1.01 * tan_fov) + 1e-9 : INFINITY;
+}
+
+// K: the POLISHED Kepler state at tm.  a: semi-major axis.  tau_max: max |t_j - tm| over the group.
+__device__ __forceinline__ GroupEph group_ephemeris(const Orbit &o, double a, const Kepler &K, double tm, double tau_max,
+                                                    double gm, double inv_c, double tan_fov)
+{
+    GroupEph G;
+    G.tm = tm;
+    const double g = fma(-o.e, K.c, 1.0);
+    const double rg = rcp_nr<2>(g);
+    const double X = K.c - o.e;
+    G.rx = fma(o.Ax, X, o.Bx * K.s);
+    G.ry = fma(o.Ay, X, o.By * K.s);
+    G.rz = fma(o.Az, X, o.Bz * K.s);
+    const double w = o.n * rg;                                   // dE/dt
+    G.vx = w * fma(o.Bx, K.c, -o.Ax * K.s);
+    G.vy = w * fma(o.By, K.c, -o.Ay * K.s);
+    G.vz = w * fma(o.Bz, K.c, -o.Az * K.s);
+    const double k = -0.5 * (o.n * o.n) * (rg * rg * rg);        // a / 2 = k r
+    G.hx = k * G.rx;
+    G.hy = k * G.ry;
+    G.hz = k * G.rz;
+    G.tq = gate_tq(o.vmax, inv_c, tan_fov);
+    // |r| over the group: no closer than the perihelion, no closer than |r(tm)| minus the longest way the object can go
+    G.eps = gate_eps_bound(gm, o.vmax, fmax(a * (1.0 - o.e), fma(-o.vmax, tau_max, a * g)), tau_max, tan_fov);
+    if (!(G.tq < 1e300) || !(G.eps < 1e300)) G.eps = INFINITY;   // no cone, or anything non-finite: keep every pair
+    return G;
+}
+
+// true: the pair cannot be a hit.  R: the observer at the exposure; t: unit vector to its tangent point.
+__device__ __forceinline__ bool group_gate_culls(const GroupEph &G, double t_exp, double Rx, double Ry, double Rz,
+                                                 double tx, double ty, double tz)
+{
+    const double tau = t_exp - G.tm;
+    const double px = fma(fma(G.hx, tau, G.vx), tau, G.rx) - Rx;
+    const double py = fma(fma(G.hy, tau, G.vy), tau, G.ry) - Ry;
+    const double pz = fma(fma(G.hz, tau, G.vz), tau, G.rz) - Rz;
+    const double r2 = fma(px, px, fma(py, py, pz * pz));
+    const double D0 = fma(px, tx, fma(py, ty, pz * tz));
+    const double w = fma(D0, G.tq, G.eps);
+    return (D0 < -G.eps) || (fma(-D0, D0, r2) > w * w);
 }
 
 }  // namespace dt

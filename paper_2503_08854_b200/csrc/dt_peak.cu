@@ -91,7 +91,9 @@ cudaError_t random_gather_probe(int64_t buffer_bytes, int hint64, double *gather
     float *buf = nullptr, *out = nullptr;
     e = cudaMalloc((void **)&buf, words * 4);
     if (e != cudaSuccess) return e;
-    const int blocks = sms * 2, threads = 1024, per = 256;
+    // a buffer that fits the L2 (<= 64 MiB) is gathered from four times as long: the L2-resident rate is the
+    // denominator of the dense gather schedule (bench.py `l2_gather_bound`)
+    const int blocks = sms * 2, threads = 1024, per = buffer_bytes <= (64ll << 20) ? 1024 : 256;
     e = cudaMalloc((void **)&out, (size_t)blocks * threads * 4);
     if (e != cudaSuccess) { cudaFree(buf); return e; }
     cudaMemsetAsync(buf, 0, words * 4, stream);

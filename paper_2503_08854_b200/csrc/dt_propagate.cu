@@ -24,11 +24,13 @@ namespace dt {
 #define DT_K1_MIN_CTAS 4           // resident CTAs per SM kernel 1 is compiled for (register budget)
 #endif
 constexpr int kMaxSubsteps = 6;    // wide sub-steps of one Kepler step before the cold solve is cheaper
+constexpr double kGateEpsMax = 0.03;   // AU: a looser remainder bound in the warp switches the group's gate off
 
 struct __align__(128) PropSmem {
     ExpRec rec[2][kGroup];                       // 8 KB: two-slot ring of exposure groups
     uint32_t stage[kWarpsPerCta][kGroup * 32];   // 4 KB per warp: [warp][hit] staged pixel offsets
     double el[kTileOrbits * 6];                  // 48 B per orbit: the tile's elements (one bulk copy)
+    double geph[12][kTileOrbits];                // 96 B per orbit: the gate's group ephemeris (GroupEph), lane-contiguous
     uint64_t full[2];
     uint64_t el_bar;
 };
@@ -39,6 +41,9 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
     constexpr bool WARM = (MODE & kModeWarm) != 0;
     constexpr bool PRECULL = (MODE & kModePrecull) != 0;
     constexpr bool DENSE = (MODE & kModeDense) != 0;
+    constexpr bool GATE = (MODE & kModeGate) != 0 && WARM && PRECULL;
+    // both variants of a unit are enqueued; the one the policy does not name has nothing to do
+    if (p.policy && (p.policy->select != 0) != GATE) return;
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     PropSmem &sm = *reinterpret_cast<PropSmem *>(smem_raw);
@@ -106,6 +111,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
     bool prev_refined = false;     // warp-uniform: the last exposure's pairs went through the refinement
     int since_sync = 0;            // warp-uniform: cull-quality steps since (sin E, cos E) were last exact
     unsigned long long n_refined = 0, n_cold = 0, n_hits = 0, n_sub = 0;
+    unsigned int n_gated = 0;      // warp-uniform: exposures of this warp the group ephemeris gate removed
 
     for (int g = g_begin; g < g_end; ++g) {
         const int slot = (g - g_begin) & 1;
@@ -120,10 +126,100 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
             since_sync = 0;
         }
 
+        bool gate_ready = false, gate_off = false;   // warp-uniform: this group's ephemeris exists / is of no use
         uint32_t bits = 0;
         int cnt = 0;          // this lane's hits in the group
         int run = 0;          // the warp's hits in the group so far (warp-uniform)
         for (int jj = 0; jj < nrec; ++jj) {
+            // ---- group ephemeris gate (dt_orbit.cuh, A25): while the warp is culling, ONE Taylor evaluation
+            // per pair decides whether any lane can be near the exposure; a run of exposures none can be near costs
+            // no Kepler step at all ----
+            if (GATE && !prev_refined && !gate_off) {
+                if (!gate_ready) {
+                    // lazily, once per group (a warp that refines every pair never gets here): mid-time and half-span
+                    // of the group's exposures, in whatever order they come
+                    double tlo = sm.rec[slot][min(lane, nrec - 1)].t, thi = tlo;
+#pragma unroll
+                    for (int d = 16; d > 0; d >>= 1) {
+                        tlo = fmin(tlo, __shfl_xor_sync(0xffffffffu, tlo, d));
+                        thi = fmax(thi, __shfl_xor_sync(0xffffffffu, thi, d));
+                    }
+                    const double tm = 0.5 * (tlo + thi);
+                    const double tau_max = fma(0.5 * (thi - tlo), 1.000001, 1e-9);
+                    const double a_orb = o.valid ? sm.el[tid * 6] : 1.0;
+                    gate_ready = true;
+                    // is the remainder bound of every lane tight enough to be of use?  Judged BEFORE the Kepler solve
+                    // from the carried state: |r| over the group is no smaller than |r| there minus the longest way
+                    // the object can go until the farthest exposure of the group (eccentric orbits next to a
+                    // perihelion fail this; their warp then runs the group without the gate, at no cost)
+                    if (have_state) {
+                        const double t_cur = fma(K.M - o.M0, rcp_nr<1>(o.n), t0);
+                        const double far = fmax(fabs(thi - t_cur), fabs(tlo - t_cur));
+                        const double rlow = fmax(a_orb * (1.0 - o.e), fma(-o.vmax, far, a_orb * fma(-o.e, K.c, 1.0)));
+                        gate_off = !__all_sync(0xffffffffu,
+                                               gate_eps_bound(p.gm, o.vmax, rlow, tau_max, p.tan_fov) < kGateEpsMax);
+                    }
+                    if (!gate_off) {
+                        // one polished Kepler solve at the mid-time (the carried state moves there: the chain stays at
+                        // most half a group away from any exposure)
+                        const double Mm = fma(o.n, tm - t0, o.M0);
+                        Kepler Km = K;
+                        bool okm = false;
+                        if (have_state) Km = kepler_warm_wide<true>(o.e, K, Mm, okm);
+                        if (!__all_sync(0xffffffffu, okm)) {
+                            Km = kepler_cold(o.e, Mm);
+                            n_cold += 1;
+                        }
+                        K = Km;
+                        have_state = true;
+                        since_sync = 0;
+                        const GroupEph G = group_ephemeris(o, a_orb, K, tm, tau_max, p.gm, p.inv_c, p.tan_fov);
+                        // the ephemeris lives in shared memory (lane-contiguous: conflict-free) and is read back at
+                        // the head of every gated run, so that its 24 registers are not live across the refinement
+                        sm.geph[0][tid] = G.tm;
+                        sm.geph[1][tid] = G.rx;
+                        sm.geph[2][tid] = G.ry;
+                        sm.geph[3][tid] = G.rz;
+                        sm.geph[4][tid] = G.vx;
+                        sm.geph[5][tid] = G.vy;
+                        sm.geph[6][tid] = G.vz;
+                        sm.geph[7][tid] = G.hx;
+                        sm.geph[8][tid] = G.hy;
+                        sm.geph[9][tid] = G.hz;
+                        sm.geph[10][tid] = G.tq;
+                        sm.geph[11][tid] = G.eps;
+                        gate_off = !__all_sync(0xffffffffu, G.eps < kGateEpsMax);
+                    }
+                }
+                if (!gate_off) {
+                    GroupEph G;
+                    G.tm = sm.geph[0][tid];
+                    G.rx = sm.geph[1][tid];
+                    G.ry = sm.geph[2][tid];
+                    G.rz = sm.geph[3][tid];
+                    G.vx = sm.geph[4][tid];
+                    G.vy = sm.geph[5][tid];
+                    G.vz = sm.geph[6][tid];
+                    G.hx = sm.geph[7][tid];
+                    G.hy = sm.geph[8][tid];
+                    G.hz = sm.geph[9][tid];
+                    G.tq = sm.geph[10][tid];
+                    G.eps = sm.geph[11][tid];
+                    const int j_first = jj;
+                    for (; jj < nrec; ++jj) {
+                        const ExpRec &y = sm.rec[slot][jj];
+                        if (__any_sync(0xffffffffu, !group_gate_culls(G, y.t, y.Rx, y.Ry, y.Rz, y.tx, y.ty, y.tz))) break;
+                        if (DENSE && in_range) {          // dt_project: a gated pair is reported as culled
+                            const int64_t k = (orbit * p.n_exp + (int64_t)g * kGroup + jj) * 2;
+                            if (p.radec) p.radec[k] = p.radec[k + 1] = nan("");
+                            if (p.xy) p.xy[k] = p.xy[k + 1] = nan("");
+                            if (p.pix) p.pix[k] = p.pix[k + 1] = -1;
+                        }
+                    }
+                    n_gated += (unsigned)(jj - j_first);
+                    if (jj >= nrec) break;
+                }
+            }
             const ExpRec &x = sm.rec[slot][jj];
             const double dt = x.t - t0;
             const double M = fma(o.n, dt, o.M0);
@@ -364,6 +460,7 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
         atomicAdd(p.counters + 2, n_cold);
         if (n_hits) atomicAdd(p.counters + 3, n_hits);
         if (n_sub) atomicAdd(p.counters + 4, n_sub);
+        if (GATE && n_gated) atomicAdd(p.counters + 6, 32ull * n_gated);   // pairs
     }
 }
 
@@ -390,8 +487,36 @@ cudaError_t launch_propagate(const PropagateParams &p, int mode, cudaStream_t st
         case 5: return launch_mode<5>(p, stream);
         case 6: return launch_mode<6>(p, stream);
         case 7: return launch_mode<7>(p, stream);
+        case 11: return launch_mode<11>(p, stream);
+        case 15: return launch_mode<15>(p, stream);
         default: return cudaErrorInvalidValue;
     }
+}
+
+// ---- which kernel-1 variant the NEXT unit runs (GatePolicy, dt_k1.cuh): one thread, after every unit ----
+// The gate pays where the warps cull (a blind search) and its remainder bounds are tight enough to gate; it costs
+// where most pairs are refined anyway (a focused search: the variant without it is the faster binary there) or where
+// the bounds are loose (eccentric near-Earth orbits).  Both are read off what the unit just did.
+__global__ void k_gate_policy(GatePolicy *pol, const unsigned long long *counters, long long unit_pairs)
+{
+    const unsigned long long refined = counters[1] - pol->refined0, gated = counters[6] - pol->gated0;
+    pol->refined0 = counters[1];
+    pol->gated0 = counters[6];
+    int cooldown = pol->cooldown;
+    const bool culling = (long long)refined * 4 < unit_pairs;
+    if (pol->select != 0 && culling && (long long)gated * 4 < unit_pairs)
+        cooldown = 64;                                   // the gate ran and gated little: off, tried again in 64 units
+    else if (cooldown > 0)
+        cooldown -= 1;
+    pol->cooldown = cooldown;
+    pol->select = (culling && cooldown == 0) ? 1 : 0;
+}
+
+cudaError_t launch_gate_policy(GatePolicy *policy, const unsigned long long *counters, int64_t unit_pairs,
+                               cudaStream_t stream)
+{
+    k_gate_policy<<<1, 1, 0, stream>>>(policy, counters, (long long)unit_pairs);
+    return cudaGetLastError();
 }
 
 template <int MODE>
@@ -411,7 +536,9 @@ cudaError_t init_propagate_kernels()
     if ((e = set_smem_attr<4>()) != cudaSuccess) return e;
     if ((e = set_smem_attr<5>()) != cudaSuccess) return e;
     if ((e = set_smem_attr<6>()) != cudaSuccess) return e;
-    return set_smem_attr<7>();
+    if ((e = set_smem_attr<7>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<11>()) != cudaSuccess) return e;
+    return set_smem_attr<15>();
 }
 
 }  // namespace dt

@@ -5,11 +5,13 @@ the measured DFMA rate.  The per-pair count depends on the binary AND on the wor
 (cull-quality step, wide step, sub-steps, cold solve, refinement), so it is MEASURED, per workload, with
 
     ncu --metrics smsp__inst_executed_pipe_fp64.sum,smsp__inst_executed.sum,gpu__time_duration.sum \
-        --clock-control none -k regex:k_propagate --csv --log-file gpurun_out/k1_<workload>.csv \
-        python bench.py --count-k1 <workload>
+        --clock-control none --profile-from-start off -k regex:k_propagate --csv \
+        --log-file gpurun_out/k1_<workload>.csv python bench.py --count-k1 <workload>
 
-(`--count-k1` runs ONE dt_stack of the workload at a reduced orbit count -- same seeded distributions, so the
-same mix -- and writes the pair count to gpurun_out/k1_<workload>.txt) and stored by
+(`--count-k1` runs kernel 1 over all exposures of the workload at a reduced orbit count -- same seeded distributions,
+so the same mix -- twice: an unprofiled pass in which the device-side choice of the kernel-1 variant settles, then the
+counted pass after cudaProfilerStart; both variants of a unit are launched and the one not chosen returns at once, so
+the sums hold what really ran; the pair count goes to gpurun_out/k1_<workload>.txt) and stored by
 
     python -m paper_2503_08854_b200.k1_counts gpurun_out/k1_*.csv
 

@@ -655,3 +655,115 @@ def test_precull_is_conservative_at_scale(case):
     if not case.endswith("+focused"):
         assert out[0][3] < 0.05 * out[4][3]      # and it does cull
     print(case, "hits", out[0][2], "refined pairs with / without the pre-cull", out[0][3], out[4][3])
+
+
+# ---- group ephemeris gate (reading A25) ----------------------------------------------------------------------
+GATE_CASES = {
+    # full cadence (the gate's remainder bound grows with the cube of a group's half-span, so the reduced
+    # exposure counts of CASES would switch it off), reduced planes and orbit counts; (base, overrides, guides)
+    "mba": ("small_mba", dict(n_orbits=4096, width=512, height=384), 24),
+    "lsst": ("lsst", dict(n_orbits=3072, n_exp=1200, width=320, height=256), 24),
+    "neo": ("neo", dict(n_orbits=4096, width=512, height=512), 24),
+    "tno": ("tno", dict(n_orbits=3072, width=320, height=320), 4),
+}
+
+
+def _gate_scene(case):
+    """A focused search whose orbits are re-ordered so that every warp tile of 32 holds members of ONE family (then
+    the diffuse orbits): at the exposures that follow another guide all 32 lanes are far and the gate decides for the
+    whole warp; at the exposures of the tile's own guide all 32 sit inside or at the edge of the footprint at once."""
+    base, kw, n_guides = GATE_CASES[case]
+    cfg = ds.focused(ds.scaled(ds.CONFIGS[base], **kw), n_guides=n_guides)
+    sc = ds.build_scene(cfg, oracle.scene_project_fn)
+    el = sc.elements()
+    guides = ds.workloads.guide_elements(cfg)
+    d = np.abs(el[:, None, :] - guides[None, :, :]).max(-1)
+    fam, member = d.argmin(-1), d.min(-1) < 0.05
+    order = np.concatenate([np.flatnonzero(member & (fam == g)) for g in range(guides.shape[0])] +
+                           [np.flatnonzero(~member)])
+    return sc, np.ascontiguousarray(el[order])
+
+
+@pytest.mark.parametrize("case", list(GATE_CASES))
+def test_group_gate_against_oracle(case):
+    """The gate must never remove a pair the oracle reports as a hit, whatever it does to the others, and the pairs
+    that reach the per-pair path keep full precision (dt_project under DT_FLAG_PROJECT_PRECULL = kernel 1 exactly
+    as dt_stack runs it, gate included; flags 24 = the same without the gate)."""
+    dt = _dt()
+    sc, el = _gate_scene(case)
+    el = el[:2048]
+    ref = oracle.project(oracle.Survey.from_scene(sc), el, sc.t0)
+    ohit = ref["pix"][..., 0] >= 0
+    fr = {}
+    for flags in (8, 24):
+        with dt.Tracker.from_scene(sc, flags=flags) as trk:
+            out = trk.project(el, sc.t0)
+        refined = np.isfinite(out["radec"][..., 0])
+        assert not (ohit & ~refined).any(), (flags, np.argwhere(ohit & ~refined)[:5])
+        assert (out["pix"][~refined] == -1).all()
+        sub = dict(radec=np.where(refined[..., None], out["radec"], ref["radec"]),
+                   xy=np.where(refined[..., None], out["xy"], ref["xy"]),
+                   pix=np.where(refined[..., None], out["pix"], ref["pix"]))
+        _compare_project(sub, ref)
+        fr[flags] = float(refined.mean())
+    assert int(ohit.sum()) > 100, "no hits: the test would be vacuous"
+    assert fr[8] <= fr[24] + 1e-12
+    parity_record("group_gate_project[%s]" % case, pairs=int(ohit.size), oracle_hits=int(ohit.sum()),
+                  refined_fraction_gate=fr[8], refined_fraction_no_gate=fr[24])
+
+
+@pytest.mark.parametrize("case", list(GATE_CASES))
+def test_group_gate_changes_nothing(case):
+    """dt_stack with the gate forced on, switched off, and chosen on the device: SNR and hit counts are bit-identical
+    (the gate only removes pairs that are no hits), and where its bounds are tight it really removes most of the
+    per-pair Kepler steps of these searches."""
+    dt = _dt()
+    sc, el = _gate_scene(case)
+    flux, var = _planes(sc, sc.cfg.variance_mode)
+    res = {}
+    for gate in (1, 0, -1):
+        with dt.Tracker.from_scene(sc) as trk:
+            trk.set_option("group_gate", gate)
+            trk.load_image_batch(0, flux, var)
+            snr, hits = trk.stack(el, sc.t0)
+            res[gate] = (np.array(snr), np.array(hits), trk.stats())
+    for gate in (0, -1):
+        assert np.array_equal(res[1][1], res[gate][1])
+        assert np.array_equal(res[1][0], res[gate][0], equal_nan=True)
+        assert res[1][2]["hits"] == res[gate][2]["hits"]
+    st = res[1][2]
+    assert res[0][2]["gated_pairs"] == 0 and st["hits"] > 100
+    frac = st["gated_pairs"] / st["pairs"]
+    if case != "neo":                      # eccentric near-Earth orbits: the bounds are loose next to a perihelion
+        assert frac > 0.5, frac
+    parity_record("group_gate_stack[%s]" % case, pairs=int(st["pairs"]), hits=int(st["hits"]),
+                  gated_fraction=frac, gated_fraction_device_choice=res[-1][2]["gated_pairs"] / st["pairs"],
+                  refined_fraction=st["refined_pairs"] / st["pairs"],
+                  refined_fraction_no_gate=res[0][2]["refined_pairs"] / res[0][2]["pairs"])
+
+
+def test_group_gate_device_choice():
+    """The device-side policy: a blind search (every warp culls) keeps the gate from unit to unit; a focused search
+    with mixed warps (most pairs refined) drops it after its first unit.  Results equal the gate-less run."""
+    dt = _dt()
+    out = {}
+    for name, foc in (("blind", False), ("focused", True)):
+        cfg = ds.scaled(ds.CONFIGS["lsst"], n_orbits=8192, width=160, height=128)       # 2000 exposures: 4 units
+        if foc:
+            cfg = ds.focused(cfg)
+        sc = ds.build_scene(cfg, oracle.scene_project_fn)
+        flux, var = _planes(sc, cfg.variance_mode)
+        el = sc.elements()
+        runs = {}
+        for flags in (0, 16):
+            with dt.Tracker.from_scene(sc, flags=flags) as trk:
+                trk.load_image_batch(0, flux, var)
+                snr, hits = trk.stack(el, sc.t0)
+                runs[flags] = (np.array(snr), np.array(hits), trk.stats())
+        assert np.array_equal(runs[0][1], runs[16][1]) and np.array_equal(runs[0][0], runs[16][0], equal_nan=True)
+        st = runs[0][2]
+        out[name] = st["gated_pairs"] / st["pairs"]
+        assert st["launches"] == 3 * st["propagate_launches"] + st["gather_launches"] + 1
+    assert out["blind"] > 0.8, out                  # all four units gated
+    assert out["focused"] < 0.3, out                # at most the first of four units ran the gate variant
+    parity_record("group_gate_device_choice", gated_fraction=out)
