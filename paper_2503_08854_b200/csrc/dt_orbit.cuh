@@ -31,6 +31,7 @@ struct Orbit {
     double cos2_cull;               // cos^2 of the pre-cull cone half-angle
     double rho2_close;              // pairs closer than this (AU^2) are always refined
     double vmax;                    // perihelion speed, AU / day (the largest speed on the orbit)
+    double inv_n;                   // 1 / n
     bool valid;
 };
 
@@ -53,6 +54,7 @@ __device__ __forceinline__ Orbit orbit_setup(const double el_in[6], double gm, d
     if (!o.valid) { el[0] = 1.0; el[1] = 0.0; el[2] = el[3] = el[4] = el[5] = 0.0; }
     const double a = el[0], e = el[1];
     o.n = sqrt(gm / (a * a * a));
+    o.inv_n = 1.0 / o.n;
     o.e = e;
     o.M0 = el[5];
     double si, ci, sO, cO, sw, cw;
@@ -507,11 +509,21 @@ __device__ __forceinline__ Kepler kepler_refresh(double e, const Kepler &K0)
 // pair unless D0 < -eps or d0 > D0 tq + eps, with tq and eps below (5 % margins on every term; comparisons are
 // written so that a NaN keeps the pair).  Nothing else changes: a pair the gate keeps goes through the cull-quality
 // chain and the exact cone test as before, from a Kepler state that is at most half a group old.
+// The per-pair test runs in FP32 -- it is a filter with explicit margins, not a result -- so that it costs FP32-pipe
+// issue slots instead of FP64 ones.  Its rounding enters the bound like everything else T2 leaves out.  With u = 2^-24:
+//   * the FP32 vector p~ = fl(fl(fma(fl(fma(h~, tau~, v~)), tau~, r~)) - R~) from inputs rounded to FP32 differs from
+//     T2 - R_obs by <= 6 u A per component, A = |r| + |v| tau_max + |a/2| tau_max^2 + max |R_obs| (three roundings of
+//     the inputs and two of the operations on each term at most); 24 u A (2.3 x the vector norm of that) is added to
+//     the displacement bound epsT, so p~ takes the place of T2 - R_obs in the derivation above;
+//   * D~ = fl(p~ . t~) is off by <= 6 u |p~| and r2~ = fl(p~ . p~) by <= 3 u |p~|^2, hence fma(-D~, D~, r2~) differs
+//     from |p~|^2 - (p~ . t)^2 by <= 16 u |p~|^2: the test compares it with w^2 + 40 u r2~, w = D~ tq + eps with tq
+//     and eps rounded UP after a factor (1 + 32 u) that covers the roundings of w itself and of D~ inside it.
+//     (On the far side, D~ < -eps can only be reached by vectors with |p~| <= 1.5 eps, where 6 u |p~| << 32 u eps.)
 struct GroupEph {
-    double tm;                                      // expansion time, days
-    double rx, ry, rz, vx, vy, vz, hx, hy, hz;      // r, v, a / 2 at tm: heliocentric equatorial, AU and days
-    double tq, eps;                                 // keep unless D0 < -eps or d0 > D0 tq + eps
+    float rx, ry, rz, vx, vy, vz, hx, hy, hz;       // r, v, a / 2 at the expansion time tm: heliocentric equatorial
+    float tq, eps;                                  // keep unless D0 < -eps or d0 > D0 tq + eps (+ rounding slack)
 };
+constexpr float kGateU = 5.9604645e-8f;             // 2^-24
 
 // The gate's two constants.  rmin: a lower bound of |r| over the group.  MUFU seeds + one Newton / Goldschmidt step
 // (1e-12 relative) are plenty under 5 % margins.
@@ -529,45 +541,51 @@ __device__ __forceinline__ double gate_tq(double vmax, double inv_c, double tan_
     return (kap < 0.01) ? fma(kap, 1.0 + tan_fov, 1.01 * tan_fov) + 1e-9 : INFINITY;
 }
 
-// K: the POLISHED Kepler state at tm.  a: semi-major axis.  tau_max: max |t_j - tm| over the group.
-__device__ __forceinline__ GroupEph group_ephemeris(const Orbit &o, double a, const Kepler &K, double tm, double tau_max,
-                                                    double gm, double inv_c, double tan_fov)
+// K: the POLISHED Kepler state at tm.  a: semi-major axis.  tau_max: max |t_j - tm| over the group.  r_obs_max: an
+// upper bound of the observer's heliocentric distance over the group.
+__device__ __forceinline__ GroupEph group_ephemeris(const Orbit &o, double a, const Kepler &K, double tau_max,
+                                                    double r_obs_max, double gm, double inv_c, double tan_fov)
 {
     GroupEph G;
-    G.tm = tm;
     const double g = fma(-o.e, K.c, 1.0);
     const double rg = rcp_nr<2>(g);
     const double X = K.c - o.e;
-    G.rx = fma(o.Ax, X, o.Bx * K.s);
-    G.ry = fma(o.Ay, X, o.By * K.s);
-    G.rz = fma(o.Az, X, o.Bz * K.s);
+    G.rx = __double2float_rn(fma(o.Ax, X, o.Bx * K.s));
+    G.ry = __double2float_rn(fma(o.Ay, X, o.By * K.s));
+    G.rz = __double2float_rn(fma(o.Az, X, o.Bz * K.s));
     const double w = o.n * rg;                                   // dE/dt
-    G.vx = w * fma(o.Bx, K.c, -o.Ax * K.s);
-    G.vy = w * fma(o.By, K.c, -o.Ay * K.s);
-    G.vz = w * fma(o.Bz, K.c, -o.Az * K.s);
+    G.vx = __double2float_rn(w * fma(o.Bx, K.c, -o.Ax * K.s));
+    G.vy = __double2float_rn(w * fma(o.By, K.c, -o.Ay * K.s));
+    G.vz = __double2float_rn(w * fma(o.Bz, K.c, -o.Az * K.s));
     const double k = -0.5 * (o.n * o.n) * (rg * rg * rg);        // a / 2 = k r
-    G.hx = k * G.rx;
-    G.hy = k * G.ry;
-    G.hz = k * G.rz;
-    G.tq = gate_tq(o.vmax, inv_c, tan_fov);
+    G.hx = __double2float_rn(k * fma(o.Ax, X, o.Bx * K.s));
+    G.hy = __double2float_rn(k * fma(o.Ay, X, o.By * K.s));
+    G.hz = __double2float_rn(k * fma(o.Az, X, o.Bz * K.s));
+    const double r = a * g;
+    const double tq = gate_tq(o.vmax, inv_c, tan_fov);
     // |r| over the group: no closer than the perihelion, no closer than |r(tm)| minus the longest way the object can go
-    G.eps = gate_eps_bound(gm, o.vmax, fmax(a * (1.0 - o.e), fma(-o.vmax, tau_max, a * g)), tau_max, tan_fov);
-    if (!(G.tq < 1e300) || !(G.eps < 1e300)) G.eps = INFINITY;   // no cone, or anything non-finite: keep every pair
+    double eps = gate_eps_bound(gm, o.vmax, fmax(a * (1.0 - o.e), fma(-o.vmax, tau_max, r)), tau_max, tan_fov);
+    // the FP32 evaluation of the vector (see above): |v| <= vmax, |a / 2| = -k r
+    const double A = r + o.vmax * tau_max + (-k * r) * (tau_max * tau_max) + r_obs_max;
+    eps = fma(24.0 * (double)kGateU * A, 1.0 + tan_fov, eps);
+    if (!(tq < 1e30) || !(eps < 1e30)) eps = INFINITY;           // no cone, or anything non-finite: keep every pair
+    G.tq = __double2float_ru(tq * (1.0 + 32.0 * (double)kGateU));
+    G.eps = __double2float_ru(eps * (1.0 + 32.0 * (double)kGateU));
     return G;
 }
 
-// true: the pair cannot be a hit.  R: the observer at the exposure; t: unit vector to its tangent point.
-__device__ __forceinline__ bool group_gate_culls(const GroupEph &G, double t_exp, double Rx, double Ry, double Rz,
-                                                 double tx, double ty, double tz)
+// true: the pair cannot be a hit.  tau = t_exposure - tm, R the observer at the exposure, t the unit vector to its
+// tangent point, all rounded to FP32.  A NaN keeps the pair.
+__device__ __forceinline__ bool group_gate_culls(const GroupEph &G, float tau, float Rx, float Ry, float Rz, float tx,
+                                                 float ty, float tz)
 {
-    const double tau = t_exp - G.tm;
-    const double px = fma(fma(G.hx, tau, G.vx), tau, G.rx) - Rx;
-    const double py = fma(fma(G.hy, tau, G.vy), tau, G.ry) - Ry;
-    const double pz = fma(fma(G.hz, tau, G.vz), tau, G.rz) - Rz;
-    const double r2 = fma(px, px, fma(py, py, pz * pz));
-    const double D0 = fma(px, tx, fma(py, ty, pz * tz));
-    const double w = fma(D0, G.tq, G.eps);
-    return (D0 < -G.eps) || (fma(-D0, D0, r2) > w * w);
+    const float px = fmaf(fmaf(G.hx, tau, G.vx), tau, G.rx) - Rx;
+    const float py = fmaf(fmaf(G.hy, tau, G.vy), tau, G.ry) - Ry;
+    const float pz = fmaf(fmaf(G.hz, tau, G.vz), tau, G.rz) - Rz;
+    const float r2 = fmaf(px, px, fmaf(py, py, pz * pz));
+    const float D0 = fmaf(px, tx, fmaf(py, ty, pz * tz));
+    const float w = fmaf(D0, G.tq, G.eps);
+    return (D0 < -G.eps) || (fmaf(-D0, D0, r2) > fmaf(w, w, 40.0f * kGateU * r2));
 }
 
 }  // namespace dt

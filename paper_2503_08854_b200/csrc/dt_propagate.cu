@@ -23,6 +23,9 @@ namespace dt {
 #ifndef DT_K1_MIN_CTAS
 #define DT_K1_MIN_CTAS 4           // resident CTAs per SM kernel 1 is compiled for (register budget)
 #endif
+#ifndef DT_K1_GATE_CTAS
+#define DT_K1_GATE_CTAS 5          // the gate variant: its hot loop is latency-bound, one more CTA per SM pays
+#endif
 constexpr int kMaxSubsteps = 6;    // wide sub-steps of one Kepler step before the cold solve is cheaper
 constexpr double kGateEpsMax = 0.03;   // AU: a looser remainder bound in the warp switches the group's gate off
 
@@ -30,13 +33,16 @@ struct __align__(128) PropSmem {
     ExpRec rec[2][kGroup];                       // 8 KB: two-slot ring of exposure groups
     uint32_t stage[kWarpsPerCta][kGroup * 32];   // 4 KB per warp: [warp][hit] staged pixel offsets
     double el[kTileOrbits * 6];                  // 48 B per orbit: the tile's elements (one bulk copy)
-    double geph[12][kTileOrbits];                // 96 B per orbit: the gate's group ephemeris (GroupEph), lane-contiguous
+    float geph[11][kTileOrbits];                 // 44 B per orbit: the gate's group ephemeris (GroupEph), lane-contiguous
+    float4 gexp[kWarpsPerCta][kGroup][2];        // 1 KB per warp: the group's exposures as the gate reads them, FP32:
+                                                 // (t - tm, Rx, Ry, Rz), (tx, ty, tz, -)
     uint64_t full[2];
     uint64_t el_bar;
 };
 
 template <int MODE>
-__global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const PropagateParams p)
+__global__ void __launch_bounds__(kTileOrbits, (MODE & kModeGate) ? DT_K1_GATE_CTAS : DT_K1_MIN_CTAS)
+    k_propagate(const PropagateParams p)
 {
     constexpr bool WARM = (MODE & kModeWarm) != 0;
     constexpr bool PRECULL = (MODE & kModePrecull) != 0;
@@ -138,14 +144,20 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                 if (!gate_ready) {
                     // lazily, once per group (a warp that refines every pair never gets here): mid-time and half-span
                     // of the group's exposures, in whatever order they come
-                    double tlo = sm.rec[slot][min(lane, nrec - 1)].t, thi = tlo;
-#pragma unroll
-                    for (int d = 16; d > 0; d >>= 1) {
-                        tlo = fmin(tlo, __shfl_xor_sync(0xffffffffu, tlo, d));
-                        thi = fmax(thi, __shfl_xor_sync(0xffffffffu, thi, d));
-                    }
+                    // (any expansion time will do and the half-span only has to be an upper bound: FP32 offsets from
+                    // the group's first record, reduced with two integer warp reductions on order-preserving keys)
+                    const double t_first = sm.rec[slot][0].t;
+                    const float off = __double2float_rn(sm.rec[slot][min(lane, nrec - 1)].t - t_first);
+                    const uint32_t ob = __float_as_uint(off);
+                    const uint32_t okey = ob ^ ((uint32_t)((int32_t)ob >> 31) | 0x80000000u);
+                    const uint32_t klo = __reduce_min_sync(0xffffffffu, okey), khi = __reduce_max_sync(0xffffffffu, okey);
+                    const float flo = __uint_as_float(klo ^ (((klo >> 31) - 1u) | 0x80000000u));
+                    const float fhi = __uint_as_float(khi ^ (((khi >> 31) - 1u) | 0x80000000u));
+                    const double tlo = t_first + (double)flo, thi = t_first + (double)fhi;
                     const double tm = 0.5 * (tlo + thi);
-                    const double tau_max = fma(0.5 * (thi - tlo), 1.000001, 1e-9);
+                    // + the rounding of the offsets (2^-24 relative each)
+                    const double tau_max = fma(0.5 * (thi - tlo) + 1.2e-7 * fmax(fabs((double)flo), fabs((double)fhi)),
+                                               1.000001, 1e-9);
                     const double a_orb = o.valid ? sm.el[tid * 6] : 1.0;
                     gate_ready = true;
                     // is the remainder bound of every lane tight enough to be of use?  Judged BEFORE the Kepler solve
@@ -153,13 +165,26 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                     // the object can go until the farthest exposure of the group (eccentric orbits next to a
                     // perihelion fail this; their warp then runs the group without the gate, at no cost)
                     if (have_state) {
-                        const double t_cur = fma(K.M - o.M0, rcp_nr<1>(o.n), t0);
+                        const double t_cur = fma(K.M - o.M0, o.inv_n, t0);
                         const double far = fmax(fabs(thi - t_cur), fabs(tlo - t_cur));
                         const double rlow = fmax(a_orb * (1.0 - o.e), fma(-o.vmax, far, a_orb * fma(-o.e, K.c, 1.0)));
                         gate_off = !__all_sync(0xffffffffu,
                                                gate_eps_bound(p.gm, o.vmax, rlow, tau_max, p.tan_fov) < kGateEpsMax);
                     }
                     if (!gate_off) {
+                        // lane j turns exposure j into what the test reads, FP32 (the warp's own copy: no CTA barrier)
+                        float robs2 = 0.f;
+                        if (lane < nrec) {
+                            const ExpRec &y = sm.rec[slot][lane];
+                            sm.gexp[warp][lane][0] = make_float4(__double2float_rn(y.t - tm), __double2float_rn(y.Rx),
+                                                                 __double2float_rn(y.Ry), __double2float_rn(y.Rz));
+                            sm.gexp[warp][lane][1] = make_float4(__double2float_rn(y.tx), __double2float_rn(y.ty),
+                                                                 __double2float_rn(y.tz), 0.f);
+                            robs2 = __double2float_ru(fma(y.Rx, y.Rx, fma(y.Ry, y.Ry, y.Rz * y.Rz)));
+                        }
+                        // max over the group (non-negative floats order like their bit patterns)
+                        robs2 = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(robs2)));
+                        const double r_obs_max = 1.000001 * sqrt((double)robs2);
                         // one polished Kepler solve at the mid-time (the carried state moves there: the chain stays at
                         // most half a group away from any exposure)
                         const double Mm = fma(o.n, tm - t0, o.M0);
@@ -173,48 +198,61 @@ __global__ void __launch_bounds__(kTileOrbits, DT_K1_MIN_CTAS) k_propagate(const
                         K = Km;
                         have_state = true;
                         since_sync = 0;
-                        const GroupEph G = group_ephemeris(o, a_orb, K, tm, tau_max, p.gm, p.inv_c, p.tan_fov);
+                        const GroupEph G = group_ephemeris(o, a_orb, K, tau_max, r_obs_max, p.gm, p.inv_c, p.tan_fov);
                         // the ephemeris lives in shared memory (lane-contiguous: conflict-free) and is read back at
-                        // the head of every gated run, so that its 24 registers are not live across the refinement
-                        sm.geph[0][tid] = G.tm;
-                        sm.geph[1][tid] = G.rx;
-                        sm.geph[2][tid] = G.ry;
-                        sm.geph[3][tid] = G.rz;
-                        sm.geph[4][tid] = G.vx;
-                        sm.geph[5][tid] = G.vy;
-                        sm.geph[6][tid] = G.vz;
-                        sm.geph[7][tid] = G.hx;
-                        sm.geph[8][tid] = G.hy;
-                        sm.geph[9][tid] = G.hz;
-                        sm.geph[10][tid] = G.tq;
-                        sm.geph[11][tid] = G.eps;
-                        gate_off = !__all_sync(0xffffffffu, G.eps < kGateEpsMax);
+                        // the head of every gated run, so that its registers are not live across the refinement
+                        sm.geph[0][tid] = G.rx;
+                        sm.geph[1][tid] = G.ry;
+                        sm.geph[2][tid] = G.rz;
+                        sm.geph[3][tid] = G.vx;
+                        sm.geph[4][tid] = G.vy;
+                        sm.geph[5][tid] = G.vz;
+                        sm.geph[6][tid] = G.hx;
+                        sm.geph[7][tid] = G.hy;
+                        sm.geph[8][tid] = G.hz;
+                        sm.geph[9][tid] = G.tq;
+                        sm.geph[10][tid] = G.eps;
+                        gate_off = !__all_sync(0xffffffffu, G.eps < (float)kGateEpsMax);
+                        __syncwarp();
                     }
                 }
                 if (!gate_off) {
                     GroupEph G;
-                    G.tm = sm.geph[0][tid];
-                    G.rx = sm.geph[1][tid];
-                    G.ry = sm.geph[2][tid];
-                    G.rz = sm.geph[3][tid];
-                    G.vx = sm.geph[4][tid];
-                    G.vy = sm.geph[5][tid];
-                    G.vz = sm.geph[6][tid];
-                    G.hx = sm.geph[7][tid];
-                    G.hy = sm.geph[8][tid];
-                    G.hz = sm.geph[9][tid];
-                    G.tq = sm.geph[10][tid];
-                    G.eps = sm.geph[11][tid];
+                    G.rx = sm.geph[0][tid];
+                    G.ry = sm.geph[1][tid];
+                    G.rz = sm.geph[2][tid];
+                    G.vx = sm.geph[3][tid];
+                    G.vy = sm.geph[4][tid];
+                    G.vz = sm.geph[5][tid];
+                    G.hx = sm.geph[6][tid];
+                    G.hy = sm.geph[7][tid];
+                    G.hz = sm.geph[8][tid];
+                    G.tq = sm.geph[9][tid];
+                    G.eps = sm.geph[10][tid];
                     const int j_first = jj;
-                    for (; jj < nrec; ++jj) {
-                        const ExpRec &y = sm.rec[slot][jj];
-                        if (__any_sync(0xffffffffu, !group_gate_culls(G, y.t, y.Rx, y.Ry, y.Rz, y.tx, y.ty, y.tz))) break;
-                        if (DENSE && in_range) {          // dt_project: a gated pair is reported as culled
-                            const int64_t k = (orbit * p.n_exp + (int64_t)g * kGroup + jj) * 2;
-                            if (p.radec) p.radec[k] = p.radec[k + 1] = nan("");
-                            if (p.xy) p.xy[k] = p.xy[k + 1] = nan("");
-                            if (p.pix) p.pix[k] = p.pix[k + 1] = -1;
+                    // four exposures per step: independent dependency chains per lane, one loop overhead
+                    bool stop = false;
+                    while (!stop && jj < nrec) {
+                        unsigned kept = 0;                 // bit q: some lane may be near exposure jj + q
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            const int jq = min(jj + q, nrec - 1);
+                            const float4 a = sm.gexp[warp][jq][0], b = sm.gexp[warp][jq][1];
+                            const bool keep = !group_gate_culls(G, a.x, a.y, a.z, a.w, b.x, b.y, b.z);
+                            kept |= (__ballot_sync(0xffffffffu, keep) != 0u ? 1u : 0u) << q;
                         }
+                        const int valid = min(4, nrec - jj);
+                        const int adv = min(kept ? __ffs(kept) - 1 : 4, valid);      // exposures gated by this step
+                        stop = adv < valid;
+                        if (DENSE && in_range) {          // dt_project: a gated pair is reported as culled
+                            for (int q = 0; q < adv; ++q) {
+                                const int64_t k = (orbit * p.n_exp + (int64_t)g * kGroup + jj + q) * 2;
+                                if (p.radec) p.radec[k] = p.radec[k + 1] = nan("");
+                                if (p.xy) p.xy[k] = p.xy[k + 1] = nan("");
+                                if (p.pix) p.pix[k] = p.pix[k + 1] = -1;
+                            }
+                        }
+                        jj += adv;
                     }
                     n_gated += (unsigned)(jj - j_first);
                     if (jj >= nrec) break;
