@@ -363,7 +363,10 @@ def unit_hit_list(w, n_unit=UNIT_ORBITS):
     dev, cfg = w.dev, w.cfg
     n = min(w.n, n_unit)
     ne = min(cfg.n_exp, UNIT_EXPOSURES)
-    hl = w.trk.filter_intersections(w.el_dev[:n], w.scene.t0, 0, ne)
+    # in the order dt_stack processes the unit in (sky order, csrc/dt_sort.cu): the list kernel 3 really gets
+    el_unit = w.el_dev[:n]
+    el_unit = el_unit[w.trk.sky_order(el_unit, w.scene.t0)].contiguous()
+    hl = w.trk.filter_intersections(el_unit, w.scene.t0, 0, ne)
     G, n_pad = hl["n_groups"], hl["n_pad"]
     words = 2 if cfg.variance_mode == 1 else 1                     # fp32 words per pixel in the resident store
     px_per_sector = 8 // words
@@ -681,6 +684,7 @@ def main():
         el = elements_device(cfg, 0, cfg.n_orbits, dev)
         st = {"pairs": 0, "hits": 0, "propagate_launches": 0}
         with dt.Tracker.from_scene(scene, device=local_rank, flags=args.flags) as trk:      # kernel 1 needs no images
+            el = el[trk.sky_order(el, scene.t0)].contiguous()        # the order dt_stack processes the unit in
             # pass 0, unprofiled (the ncu command says --profile-from-start off): the device-side choice of the
             # kernel-1 variant settles, as it has for all but the first of a full step's ~100 units; pass 1 is counted
             for counted in (False, True):

@@ -317,7 +317,24 @@ int dt_filter_intersections(dt_context *ctx, const double *elements, int64_t n, 
                             int32_t *n_groups);
 
 /*
+ * dt_sky_order: the order dt_stack processes one unit of orbits in (option "sort_orbits"; csrc/dt_sort.cu): position i
+ * of the sorted unit holds orbit perm_out[i].  elements [n][6] fp64 and t0_orbit [n] (or NULL: the scalar t0) are
+ * DEVICE arrays, n <= 2^20 (one unit), perm_out [n] uint32 a DEVICE array.  The key of an orbit is the equal-area
+ * sky cell (512 x 2048) of its geometric direction from the observer at the survey's middle exposure; the sort is
+ * stable, so the permutation is a pure function of the input.  A measurement / test entry: the kernel-1 and
+ * kernel-3 entries (dt_filter_intersections, dt_gather_hits) work on the order they are given, and a caller that
+ * wants what dt_stack runs passes them elements[perm].  Synchronises the context stream.
+ */
+int dt_sky_order(dt_context *ctx, const double *elements_dev, const double *t0_orbit_dev, int64_t n, double t0,
+                 uint32_t *perm_out_dev);
+
+/*
  * dt_set_option: tuning knobs of a context (none changes any result; defaults are the measured best).
+ *   "sort_orbits"         1 (default): dt_stack processes every unit of orbits in the order of where they are on the
+ *                         sky at the survey's middle exposure (a device-side sort; sums are returned in the
+ *                         caller's order), so that the 32 orbits of a warp are alike whatever order they were
+ *                         listed in; 0: in the caller's order.  Results agree to rounding of the pixel
+ *                         coordinates (1e-9 px), not bit for bit: which Kepler series a warp takes is a warp vote
  *   "group_gate"          -1 (default): for every work unit the device picks the kernel-1 variant with or without
  *                         the group ephemeris gate from what the previous unit did (on where warps cull -- a
  *                         blind search -- and the gate really gates; off where most pairs are refined or the

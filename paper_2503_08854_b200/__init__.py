@@ -31,7 +31,7 @@ DT_NOALLOC_MAX_ORBITS = 1 << 20
 EXPORTS = ["dt_create", "dt_destroy", "dt_load_image_batch", "dt_stack", "dt_stack_epochs", "dt_set_patch",
            "dt_set_outlier_clip", "dt_threshold", "dt_threshold_noalloc", "dt_partials_sparse", "dt_partials_reset", "dt_partials_add",
            "dt_partials_finalize", "dt_topk", "dt_project",
-           "dt_gather_hits", "dt_filter_intersections", "dt_set_option", "dt_get_stats", "dt_last_error", "dt_version", "dt_fp64_peak", "dt_probe_random_gather"]
+           "dt_gather_hits", "dt_filter_intersections", "dt_sky_order", "dt_set_option", "dt_get_stats", "dt_last_error", "dt_version", "dt_fp64_peak", "dt_probe_random_gather"]
 
 
 class DtError(RuntimeError):
@@ -92,6 +92,7 @@ def lib():
         L.dt_filter_intersections.argtypes = [vp, vp, C.c_int64, C.c_double, C.c_int32, C.c_int32, C.c_int32,
                                               C.POINTER(vp), C.POINTER(vp), C.POINTER(vp),
                                               C.POINTER(C.c_int64), C.POINTER(C.c_int64), ip]
+        L.dt_sky_order.argtypes = [vp, vp, vp, C.c_int64, C.c_double, vp]
         L.dt_set_option.argtypes = [vp, C.c_char_p, C.c_int64]
         L.dt_get_stats.argtypes = [vp, C.POINTER(dt_stats)]
         L.dt_last_error.argtypes = [vp]
@@ -258,6 +259,18 @@ def dt_threshold_noalloc(snr, hits, snr_min: float, min_hits, index_out, snr_out
                                       snr_out.data_ptr() if snr_out is not None else None, n_found.data_ptr()))
 
 
+def dt_sky_order(ctx, elements, t0=0.0):
+    """elements: torch CUDA tensor [n, 6] f64 (one unit, n <= 2^20) -> torch int64 tensor [n]: the order dt_stack
+    processes the unit in (elements[perm] is what its kernels see).  t0: scalar, or a CUDA tensor [n] of epochs."""
+    import torch
+    n = int(elements.shape[0])
+    perm = torch.empty(n, dtype=torch.int32, device=elements.device)
+    per_orbit = hasattr(t0, "shape") and len(t0.shape) > 0
+    _check(lib().dt_sky_order(ctx, elements.data_ptr(), t0.data_ptr() if per_orbit else None, n,
+                              0.0 if per_orbit else float(t0), perm.data_ptr()), ctx)
+    return perm.to(torch.int64)
+
+
 def dt_partials_sparse(ctx, n: int, device=None):
     """The orbits the context's exposure slice has hits for -> (index int64, S f64, Wt f64, hits i32), index
     ascending; torch CUDA tensors when `device` is given, else numpy arrays."""
@@ -421,6 +434,9 @@ class Tracker:
     def filter_intersections(self, elements, t0=0.0, first_exposure=0, n_exposures=None):
         ne = min(self.n_exposures - first_exposure, 512) if n_exposures is None else n_exposures
         return dt_filter_intersections(self.ctx, elements, t0, first_exposure, ne)
+
+    def sky_order(self, elements, t0=0.0):
+        return dt_sky_order(self.ctx, elements, t0)
 
     def set_option(self, name, value):
         dt_set_option(self.ctx, name, value)

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libdtrack.so")
-SOURCES = ["dt_api.cu", "dt_propagate.cu", "dt_gather.cu", "dt_gather_dense.cu", "dt_tiles.cu", "dt_topk.cu", "dt_peak.cu"]
+SOURCES = ["dt_api.cu", "dt_propagate.cu", "dt_gather.cu", "dt_gather_dense.cu", "dt_tiles.cu", "dt_topk.cu", "dt_peak.cu", "dt_sort.cu"]
 HEADERS = ["dt_common.cuh", "dt_k1.cuh", "dt_orbit.cuh", "dt_gather.cuh", "dt_tma.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--fmad=true",

@@ -62,6 +62,14 @@ struct dt_context {
     int64_t el_cap = 0;
     double *d_t0 = nullptr;                             // per-orbit epochs of dt_stack_epochs
     int64_t t0_cap = 0;
+    // sky order (dt_sort.cu): sorted copies kernels 1 and 3 work on, the permutation, the sort's scratch
+    int32_t sort_orbits = 1;                            // option "sort_orbits"
+    double *d_els = nullptr, *d_t0s = nullptr, *d_Ss = nullptr, *d_Wts = nullptr;
+    int32_t *d_cnts = nullptr;
+    uint32_t *d_perm = nullptr, *d_skey = nullptr;      // d_skey: [3][unit] keys in / keys out / index in
+    void *d_sort_tmp = nullptr;
+    int64_t els_cap = 0, t0s_cap = 0, Ss_cap = 0, Wts_cap = 0, cnts_cap = 0, perm_cap = 0, skey_cap = 0;
+    size_t sort_tmp_bytes = 0;
     // extended stack (dt_set_patch, dt_set_outlier_clip)
     int32_t patch = 1;
     double *d_patch_w = nullptr;                        // [patch * patch] or NULL (all 1)
@@ -95,6 +103,7 @@ struct dt_context {
     int64_t slot_floats = 0;
     bool zero_copy_elements = true;                     // false: copy pinned elements to the device first
     std::vector<cudaEvent_t> ev_pool;                   // timing events
+    std::vector<cudaEvent_t> ev_elem;                   // per orbit unit: its elements have arrived on the device
 
     // scratch of the dt_partials_* calls (host-memory callers)
     long long *d_pidx = nullptr;
@@ -173,6 +182,8 @@ void free_all(dt_context *c)
     cudaFree(c->d_base);
     cudaFree(c->d_offsets);
     cudaFree(c->d_counters);
+    cudaFree(c->d_els); cudaFree(c->d_t0s); cudaFree(c->d_Ss); cudaFree(c->d_Wts); cudaFree(c->d_cnts);
+    cudaFree(c->d_perm); cudaFree(c->d_skey); cudaFree(c->d_sort_tmp);
     cudaFree(c->d_policy);
     cudaFree(c->d_progress);
     cudaFree(c->tile_count);
@@ -183,6 +194,7 @@ void free_all(dt_context *c)
     cudaFree((void *)c->d_flux_ptrs);
     cudaFree((void *)c->d_var_ptrs);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->ev_elem) cudaEventDestroy(e);
     topk_free(c->topk);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
@@ -583,16 +595,35 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
     const double *d_el = elements;           // what later passes and k_finalize read
     const double *first_src = elements;      // what the first pass of kernel 1 reads
     double *copy_out = nullptr;
+    bool elements_by_unit = false;           // the elements arrive unit by unit on the copy stream (ev_elem)
     const bool aligned16 = (reinterpret_cast<uintptr_t>(elements) & 15u) == 0;
     if (mem_kind != DT_MEM_DEVICE || !aligned16) {
         CU(c, grow(c->d_el, c->el_cap, n * 6));
         d_el = c->d_el;
         void *mapped = nullptr;
-        if (mem_kind == DT_MEM_PINNED && aligned16 && c->zero_copy_elements &&
+        if (mem_kind == DT_MEM_PINNED && aligned16 && c->zero_copy_elements && !c->sort_orbits &&
             cudaHostGetDevicePointer(&mapped, const_cast<double *>(elements), 0) == cudaSuccess && mapped &&
             (reinterpret_cast<uintptr_t>(mapped) & 15u) == 0) {
             first_src = static_cast<const double *>(mapped);
             copy_out = c->d_el;
+        } else if (c->sort_orbits && mem_kind != DT_MEM_DEVICE) {
+            // sky order needs a unit's elements on the device before its kernel 1: one copy per orbit unit on the
+            // copy stream, all enqueued now, so that unit u + 1 crosses PCIe while unit u is being worked on
+            cudaGetLastError();
+            first_src = c->d_el;
+            const int64_t units = (n + unit_orb - 1) / unit_orb;
+            while ((int64_t)c->ev_elem.size() < units) {
+                cudaEvent_t e;
+                CU(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+                c->ev_elem.push_back(e);
+            }
+            for (int64_t u = 0; u < units; ++u) {
+                const int64_t o0 = u * unit_orb, no = std::min<int64_t>(unit_orb, n - o0);
+                CU(c, cudaMemcpyAsync(c->d_el + o0 * 6, elements + o0 * 6, (size_t)no * 48, cudaMemcpyHostToDevice,
+                                      c->copy_stream));
+                CU(c, cudaEventRecord(c->ev_elem[u], c->copy_stream));
+            }
+            elements_by_unit = true;
         } else {
             cudaGetLastError();
             CU(c, cudaMemcpyAsync(c->d_el, elements, (size_t)n * 48, cudaMemcpyDefault, c->stream));
@@ -619,6 +650,30 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
         cap = c->acc_cap; CU(c, grow(c->d_hits, cap, n));
         c->acc_cap = n;
     }
+    // sky order: kernels 1 and 3 work on a sorted copy of every unit, the sums come back in the caller's order
+    const bool sorted = c->sort_orbits != 0;
+    double *acc_S = c->d_S, *acc_Wt = c->d_Wt;
+    int32_t *acc_cnt = c->d_cnt;
+    if (sorted) {
+        CU(c, grow(c->d_els, c->els_cap, n * 6));
+        if (d_t0) CU(c, grow(c->d_t0s, c->t0s_cap, n));
+        CU(c, grow(c->d_Ss, c->Ss_cap, n));
+        CU(c, grow(c->d_Wts, c->Wts_cap, n));
+        CU(c, grow(c->d_cnts, c->cnts_cap, n));
+        CU(c, grow(c->d_perm, c->perm_cap, n));
+        CU(c, grow(c->d_skey, c->skey_cap, 3 * unit_orb));
+        const size_t need = sky_sort_temp_bytes(unit_orb);
+        if (need > c->sort_tmp_bytes) {
+            cudaFree(c->d_sort_tmp);
+            c->d_sort_tmp = nullptr;
+            c->sort_tmp_bytes = 0;
+            CU(c, cudaMalloc(&c->d_sort_tmp, need));
+            c->sort_tmp_bytes = need;
+        }
+        acc_S = c->d_Ss;
+        acc_Wt = c->d_Wts;
+        acc_cnt = c->d_cnts;
+    }
     CU(c, grow(c->d_mask, c->mask_cap, unit_orb * unit_groups));
     CU(c, grow(c->d_base, c->base_cap, (unit_orb / 32) * unit_groups));
     CU(c, grow(c->d_offsets, c->off_cap, unit_orb * (int64_t)unit_groups * kGroup));
@@ -631,9 +686,9 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
     int unit_idx = 0;
 
     CU(c, cudaEventRecord(c->ev_pool[0], c->stream));
-    CU(c, cudaMemsetAsync(c->d_S, 0, (size_t)n * 8, c->stream));
-    CU(c, cudaMemsetAsync(c->d_Wt, 0, (size_t)n * 8, c->stream));
-    CU(c, cudaMemsetAsync(c->d_cnt, 0, (size_t)n * 4, c->stream));
+    CU(c, cudaMemsetAsync(acc_S, 0, (size_t)n * 8, c->stream));
+    CU(c, cudaMemsetAsync(acc_Wt, 0, (size_t)n * 8, c->stream));
+    CU(c, cudaMemsetAsync(acc_cnt, 0, (size_t)n * 4, c->stream));
     CU(c, reset_counters(c));
 
     const int mode = propagate_mode(c);
@@ -694,6 +749,7 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
                 const int32_t ne = std::min<int32_t>(unit_exp_max, c->N);
                 PropagateParams p;
                 fill_common(c, p, t0);
+                if (elements_by_unit) CU(c, cudaStreamWaitEvent(c->stream, c->ev_elem[0], 0));
                 p.elements = first_src;
                 p.t0_orbit = d_t0;
                 p.n_orbits = no;
@@ -775,6 +831,18 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
             p.elements = (b == 0 ? first_src : d_el) + o0 * 6;
             p.t0_orbit = d_t0 ? d_t0 + o0 : nullptr;
             p.elements_copy = (b == 0 && copy_out) ? copy_out + o0 * 6 : nullptr;
+            if (b == 0 && elements_by_unit) CU(c, cudaStreamWaitEvent(c->stream, c->ev_elem[o0 / unit_orb], 0));
+            CU(c, cudaEventRecord(ev_at(3 * unit_idx), c->stream));
+            if (sorted) {
+                if (b == 0)       // once per orbit unit: the order of the survey's middle exposure serves every batch
+                    CU(c, sky_sort_unit(d_el + o0 * 6, d_t0 ? d_t0 + o0 : nullptr, no, t0, c->d_exp + c->N / 2, c->gm,
+                                        c->cos_eps, c->sin_eps, c->d_skey, c->d_skey + unit_orb, c->d_skey + 2 * unit_orb,
+                                        c->d_sort_tmp, c->sort_tmp_bytes, c->d_perm + o0, c->d_els + o0 * 6,
+                                        c->d_t0s + (d_t0 ? o0 : 0), c->stream));
+                p.elements = c->d_els + o0 * 6;
+                p.t0_orbit = d_t0 ? c->d_t0s + o0 : nullptr;
+                p.elements_copy = nullptr;
+            }
             p.n_orbits = no;
             p.n_pad = (no + 31) / 32 * 32;
             p.exp = c->d_exp + first;
@@ -786,7 +854,6 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
             p.counters = c->d_counters;
             // the hit counter restarts per unit so offsets index from 0
             CU(c, cudaMemsetAsync(c->d_counters, 0, sizeof(unsigned long long), c->stream));
-            CU(c, cudaEventRecord(ev_at(3 * unit_idx), c->stream));
             CU(c, launch_k1_unit(c, p, mode, &k1_launches));
             st.propagate_launches += 1;
             CU(c, cudaEventRecord(ev_at(3 * unit_idx + 1), c->stream));
@@ -852,9 +919,9 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
             }
             g.exp_all = c->d_exp;
             g.plane = c->plane;
-            g.S = c->d_S + o0;
-            g.Wt = c->d_Wt + o0;
-            g.cnt = c->d_cnt + o0;
+            g.S = acc_S + o0;
+            g.Wt = acc_Wt + o0;
+            g.cnt = acc_cnt + o0;
             g.progress = c->d_progress;
             g.window = c->gather_window;
             g.n_hits_dev = c->d_counters;            // the unit's hit allocator, final after kernel 1
@@ -875,6 +942,8 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
         }
     }
     CU(c, cudaEventRecord(c->ev_pool[2], c->stream));
+    if (sorted)
+        CU(c, sky_unsort_sums(c->d_perm, n, unit_orb, c->d_Ss, c->d_Wts, c->d_cnts, c->d_S, c->d_Wt, c->d_cnt, c->stream));
     CU(c, launch_finalize(d_el, d_t0, n, c->d_S, c->d_Wt, c->d_cnt, c->d_snr, c->d_hits, c->d_counters + 5,
                           c->stream));
     CU(c, cudaEventRecord(c->ev_pool[3], c->stream));
@@ -1275,6 +1344,30 @@ int dt_filter_intersections(dt_context *c, const double *elements, int64_t n, do
     return DT_OK;
 }
 
+int dt_sky_order(dt_context *c, const double *elements_dev, const double *t0_orbit_dev, int64_t n, double t0,
+                 uint32_t *perm_out_dev)
+{
+    if (!c) return DT_ERR_INVALID_ARG;
+    if (n < 0 || n > kMaxUnitOrbits || (n > 0 && (!elements_dev || !perm_out_dev)))
+        return fail(c, DT_ERR_INVALID_ARG, "dt_sky_order: one unit of at most %lld orbits, device arrays", (long long)kMaxUnitOrbits);
+    if (n == 0) return DT_OK;
+    CU(c, cudaSetDevice(c->device));
+    CU(c, grow(c->d_skey, c->skey_cap, 3 * kMaxUnitOrbits));
+    const size_t need = sky_sort_temp_bytes(kMaxUnitOrbits);
+    if (need > c->sort_tmp_bytes) {
+        cudaFree(c->d_sort_tmp);
+        c->d_sort_tmp = nullptr;
+        c->sort_tmp_bytes = 0;
+        CU(c, cudaMalloc(&c->d_sort_tmp, need));
+        c->sort_tmp_bytes = need;
+    }
+    CU(c, sky_sort_unit(elements_dev, t0_orbit_dev, n, t0, c->d_exp + c->N / 2, c->gm, c->cos_eps, c->sin_eps, c->d_skey,
+                        c->d_skey + kMaxUnitOrbits, c->d_skey + 2 * kMaxUnitOrbits, c->d_sort_tmp, c->sort_tmp_bytes,
+                        perm_out_dev, nullptr, nullptr, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return DT_OK;
+}
+
 int dt_set_option(dt_context *c, const char *name, int64_t value)
 {
     if (!c || !name) return DT_ERR_INVALID_ARG;
@@ -1285,6 +1378,8 @@ int dt_set_option(dt_context *c, const char *name, int64_t value)
     } else if (k == "group_gate") {
         if (value < -1 || value > 1) return fail(c, DT_ERR_INVALID_ARG, "group_gate: -1 chosen on the device, 0 off, 1 on");
         c->group_gate = (int32_t)value;
+    } else if (k == "sort_orbits") {
+        c->sort_orbits = value ? 1 : 0;
     } else if (k == "gather_window") {
         c->gather_window = value > 0 ? (int32_t)std::min<int64_t>(value, 64) : pick_gather_window(c);
     } else if (k == "gather_prefetch") {

@@ -150,6 +150,16 @@ cudaError_t threshold_noalloc_device(const double *snr, const int32_t *hits, int
                                      double *snr_out_dev, long long *n_found_dev, cudaStream_t stream);
 int64_t threshold_noalloc_max();
 
+// Sky order (dt_sort.cu): the permutation that sorts a unit's orbits by where they are on the sky at the key
+// exposure, the sorted copies kernels 1 and 3 work on, and the way back for the per-orbit sums.
+size_t sky_sort_temp_bytes(int64_t n_max);
+cudaError_t sky_sort_unit(const double *elements, const double *t0_orbit, int64_t n, double t0, const ExpRec *key_exp,
+                          double gm, double cos_eps, double sin_eps, uint32_t *keys_in, uint32_t *keys_out,
+                          uint32_t *index_in, void *temp, size_t temp_bytes, uint32_t *perm, double *elements_sorted,
+                          double *t0_sorted, cudaStream_t stream);
+cudaError_t sky_unsort_sums(const uint32_t *perm, int64_t n, int64_t unit, const double *S_s, const double *Wt_s,
+                            const int32_t *cnt_s, double *S, double *Wt, int32_t *cnt, cudaStream_t stream);
+
 // FP64 FMA issue-rate probe (dt_fp64_peak).
 cudaError_t fp64_peak_device(double *tflops, cudaStream_t stream);
 // Random 4-B gather rate over a buffer of buffer_bytes (dt_probe_random_gather).

@@ -744,10 +744,12 @@ def test_group_gate_changes_nothing(case):
 
 def test_group_gate_device_choice():
     """The device-side policy: a blind search (every warp culls) keeps the gate from unit to unit; a focused search
-    with mixed warps (most pairs refined) drops it after its first unit.  Results equal the gate-less run."""
+    whose family members are scattered over the warps (most pairs refined) drops it after its first unit -- unless
+    the orbits are put into sky order first (the default), which makes the warps of such a search homogeneous and
+    lets the gate work there too.  Results equal the gate-less run."""
     dt = _dt()
     out = {}
-    for name, foc in (("blind", False), ("focused", True)):
+    for name, foc, sort in (("blind", False, 1), ("focused_caller_order", True, 0), ("focused_sky_order", True, 1)):
         cfg = ds.scaled(ds.CONFIGS["lsst"], n_orbits=8192, width=160, height=128)       # 2000 exposures: 4 units
         if foc:
             cfg = ds.focused(cfg)
@@ -757,6 +759,7 @@ def test_group_gate_device_choice():
         runs = {}
         for flags in (0, 16):
             with dt.Tracker.from_scene(sc, flags=flags) as trk:
+                trk.set_option("sort_orbits", sort)
                 trk.load_image_batch(0, flux, var)
                 snr, hits = trk.stack(el, sc.t0)
                 runs[flags] = (np.array(snr), np.array(hits), trk.stats())
@@ -764,6 +767,44 @@ def test_group_gate_device_choice():
         st = runs[0][2]
         out[name] = st["gated_pairs"] / st["pairs"]
         assert st["launches"] == 3 * st["propagate_launches"] + st["gather_launches"] + 1
-    assert out["blind"] > 0.8, out                  # all four units gated
-    assert out["focused"] < 0.3, out                # at most the first of four units ran the gate variant
+    assert out["blind"] > 0.8, out                      # all four units gated
+    assert out["focused_caller_order"] < 0.3, out       # at most the first of four units ran the gate variant
+    assert out["focused_sky_order"] > 0.5, out
     parity_record("group_gate_device_choice", gated_fraction=out)
+
+
+@pytest.mark.parametrize("case", ["tiny_focused", "mba_focused", "neo_focused", "tno_focused", "neo_diffuse"])
+def test_sky_order_changes_nothing_but_rounding(case):
+    """dt_stack in sky order (the default) and in the caller's order: both against the oracle, and against each other
+    -- the same hit counts wherever the oracle flags no pair, SNR to 1e-9 (not bit for bit: which Kepler series a warp
+    takes is a warp vote, and the warps differ).  Per-orbit epochs travel with their orbits."""
+    dt = _dt()
+    sc = _scene(case)
+    el = sc.elements()
+    flux, var = _planes(sc, sc.cfg.variance_mode)
+    ref = oracle.stack(oracle.Survey.from_scene(sc), list(flux), list(var) if var is not None else None, el, sc.t0)
+    res = {}
+    for sort in (1, 0):
+        with dt.Tracker.from_scene(sc) as trk:
+            trk.set_option("sort_orbits", sort)
+            trk.load_image_batch(0, flux, var)
+            snr, hits = trk.stack(el, sc.t0)
+            _compare_stack(snr, hits, ref, "%s sort=%d" % (case, sort))
+            res[sort] = (np.array(snr), np.array(hits))
+            if sort == 1:
+                # per-orbit epochs, shifted by whole periods' worth of mean anomaly: M0' = M0 + n dt at t0 + dt
+                rs = np.random.RandomState(3)
+                dtv = rs.uniform(-50.0, 50.0, el.shape[0])
+                n_mot = np.sqrt(sc.gm / el[:, 0] ** 3) if hasattr(sc, "gm") else None
+                if n_mot is not None:
+                    el2 = el.copy()
+                    el2[:, 5] = el[:, 5] + n_mot * dtv
+                    snr2, hits2 = trk.stack(el2, sc.t0 + dtv)
+                    clean = ref["nflag"] == 0
+                    assert np.array_equal(np.asarray(hits2)[clean], ref["hits"][clean])
+    clean = ref["nflag"] == 0
+    assert np.array_equal(res[0][1][clean], res[1][1][clean])
+    same = clean & (res[0][1] == res[1][1])
+    a, b = res[0][0][same], res[1][0][same]
+    ok = (np.isnan(a) & np.isnan(b)) | (np.abs(a - b) <= 1e-9 * np.maximum(np.abs(b), 1e-3))
+    assert ok.all()
