@@ -137,12 +137,15 @@ __global__ void __launch_bounds__(kTileOrbits, (MODE & kModeGate) ? DT_K1_GATE_C
         int cnt = 0;          // this lane's hits in the group
         int run = 0;          // the warp's hits in the group so far (warp-uniform)
         for (int jj = 0; jj < nrec; ++jj) {
-            // ---- group ephemeris gate (dt_orbit.cuh, A25): while the warp is culling, ONE Taylor evaluation
+            // ---- group ephemeris gate (dt_orbit.cuh, A25): ONE Taylor evaluation
             // per pair decides whether any lane can be near the exposure; a run of exposures none can be near costs
             // no Kepler step at all ----
-            if (GATE && !prev_refined && !gate_off) {
+            // (once the group's ephemeris exists also right after a refined exposure: in a survey that follows several
+            // objects in turn, a warp's next exposure near its orbits is several exposures away; a warp that refines
+            // every exposure of a group never pays for the ephemeris)
+            if (GATE && !gate_off && (gate_ready || !prev_refined)) {
                 if (!gate_ready) {
-                    // lazily, once per group (a warp that refines every pair never gets here): mid-time and half-span
+                    // lazily, once per group: mid-time and half-span
                     // of the group's exposures, in whatever order they come
                     // (any expansion time will do and the half-span only has to be an upper bound: FP32 offsets from
                     // the group's first record, reduced with two integer warp reductions on order-preserving keys)
