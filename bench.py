@@ -66,6 +66,7 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-gather-bench", action="store_true")
     ap.add_argument("--gather-only", action="store_true", help="run only the kernel-3 micro-benchmarks")
+    ap.add_argument("--gather-slab", type=int, default=-1, help="dt_set_option gather_slab / gather_schedule 0 (experiments)")
     ap.add_argument("--gather-reps", type=int, default=5, help="timed repetitions per kernel-3 regime")
     ap.add_argument("--gather-regimes", default="", help="comma-separated subset of the kernel-3 regimes")
     return ap.parse_args()
@@ -719,6 +720,9 @@ def main():
             if name.endswith("+focused"):
                 cfg = ds.focused(cfg)
             w = Workload(dt, cfg, dev, local_rank, 0, 1, flags=args.flags, same_plane=True)
+            if args.gather_slab >= 0:
+                w.trk.set_option("gather_schedule", 0)
+                w.trk.set_option("gather_slab", args.gather_slab)
             u = unit_hit_list(w)
             regs.append(gather_on_unit(w, u, hbm_gbs, flush, args.gather_reps))
             w.close()

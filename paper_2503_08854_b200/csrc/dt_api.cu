@@ -84,6 +84,7 @@ struct dt_context {
     unsigned long long *d_counters = nullptr;           // [8]
     GatePolicy *d_policy = nullptr;                     // kernel-1 variant of the next unit (device-side choice)
     int32_t group_gate = -1;                            // -1 chosen on the device, 0 never, 1 always
+    int32_t gather_slab = -1;                           // walk in slabs: -1 chosen on the device, 0 never, k: always, k groups
     int *d_progress = nullptr;                          // kernel 3 lock-step counters, one per exposure of a unit
     int32_t gather_window = 1;                          // exposures the slowest and fastest CTA may be apart
     int32_t gather_lockstep = -1;                       // schedule: -1 decided on the device from the hit density
@@ -518,6 +519,46 @@ static cudaError_t launch_k1_unit(dt_context *c, PropagateParams &p, int mode, i
     return e;
 }
 
+// Kernel 3 of one unit: the dense schedule, the orbit-major walk in one launch, and the walk in slabs of exposure
+// groups (dt_gather.cuh gather_regime).  Unless options fix the choice all are enqueued and every kernel that is not
+// of the unit's regime -- read on the device from kernel 1's hit counter -- returns at once.
+static cudaError_t launch_gather_unit(const dt_context *c, const GatherParams &g_in, int32_t *launches)
+{
+    GatherParams g = g_in;
+    g.unit_groups = g.n_groups;
+    const bool ext = g.patch > 1 || g.patch_w != nullptr || isfinite(g.clip);
+    if (g.flux_ptrs || ext) g.lockstep_mode = 0;                       // as launch_gather: walk only
+    int32_t slab_opt = c->gather_slab;                                 // -1 auto, 0 never, k > 0: always, k groups
+    if (g.flux_ptrs || g.lockstep_mode == 1) slab_opt = 0;             // pixels over PCIe / dense forced: no slabs
+    const int32_t slab = slab_opt > 0 ? slab_opt : kSlabGroups;
+    if (slab_opt == 0 || slab >= g.n_groups) {
+        g.slab_mode = 0;
+        g.walk_form = 0;
+        *launches += (g.lockstep_mode < 0) ? 2 : 1;
+        return launch_gather(g, c->device, c->stream);
+    }
+    g.slab_mode = slab_opt > 0 ? 2 : -1;
+    if (slab_opt < 0 || g.lockstep_mode < 0) {                         // the one-launch walk (and the dense schedule)
+        g.walk_form = 0;
+        cudaError_t e = launch_gather(g, c->device, c->stream);
+        if (e != cudaSuccess) return e;
+        *launches += (g.lockstep_mode < 0) ? 2 : 1;
+    }
+    g.walk_form = 2;
+    g.skip_dense = 1;
+    for (int32_t g0 = 0; g0 < g.unit_groups; g0 += slab) {
+        GatherParams s = g;
+        s.n_groups = std::min<int32_t>(slab, g.unit_groups - g0);
+        s.mask = g.mask + (int64_t)g0 * g.n_pad;
+        s.base = g.base + (int64_t)g0 * (g.n_pad >> 5);
+        s.first_exposure = g.first_exposure + g0 * kGroup;
+        cudaError_t e = launch_gather(s, c->device, c->stream);
+        if (e != cudaSuccess) return e;
+        *launches += 1;
+    }
+    return cudaSuccess;
+}
+
 static void fill_gather_ext(const dt_context *c, GatherParams &g)
 {
     g.tile_capacity = c->tile_capacity;
@@ -931,8 +972,7 @@ static int stack_impl(dt_context *c, const double *elements, const double *t0_or
             g.n_exp_store = c->N;
             g.sm_count = c->sm_count;
             fill_gather_ext(c, g);
-            CU(c, launch_gather(g, c->device, c->stream));
-            st.gather_launches += (g.lockstep_mode < 0) ? 2 : 1;   // both schedules are enqueued, one of them returns at once
+            CU(c, launch_gather_unit(c, g, &st.gather_launches));
             CU(c, cudaEventRecord(ev_at(3 * unit_idx + 2), c->stream));
             unit_idx += 1;
         }
@@ -1281,7 +1321,10 @@ int dt_gather_hits(dt_context *c, int64_t n, int32_t first_exposure, int32_t n_g
 #ifdef DT_BOUNDS_CHECK
     CU(c, cudaMemsetAsync(c->d_counters + 7, 0, sizeof(unsigned long long), c->stream));
 #endif
-    CU(c, launch_gather(g, c->device, c->stream));
+    {
+        int32_t launches = 0;
+        CU(c, launch_gather_unit(c, g, &launches));
+    }
 #ifdef DT_BOUNDS_CHECK
     {
         unsigned long long bad = 0;
@@ -1380,6 +1423,8 @@ int dt_set_option(dt_context *c, const char *name, int64_t value)
         c->group_gate = (int32_t)value;
     } else if (k == "sort_orbits") {
         c->sort_orbits = value ? 1 : 0;
+    } else if (k == "gather_slab") {
+        c->gather_slab = (int32_t)std::max<int64_t>(-1, std::min<int64_t>(value, 1 << 20));
     } else if (k == "gather_window") {
         c->gather_window = value > 0 ? (int32_t)std::min<int64_t>(value, 64) : pick_gather_window(c);
     } else if (k == "gather_prefetch") {

@@ -37,6 +37,13 @@ struct GatherParams {
     const unsigned long long *n_hits_dev;   // hits of the unit on the device (kernel 1's counter) or NULL
     int64_t n_hits_host;        // used when n_hits_dev is NULL
     int32_t lockstep_mode;      // -1: decide from the hit density; 0: sparse schedule; 1: dense schedule
+    // the orbit-major walk comes in two forms: one launch over the unit's groups (regime 0), or one launch per slab
+    // of a few groups with the sums carried through S / Wt / cnt (regime 2): all warps are then within one slab of
+    // each other and a line several orbits gather from is still in the L2 when the next orbit comes by
+    int32_t slab_mode;          // -1: decide from the hit count; 0: one launch; 2: slabs
+    int32_t walk_form;          // which form THIS launch of the walk is (0 or 2): it returns at once in the other regime
+    int32_t unit_groups;        // exposure groups of the whole unit (a slab launch has fewer in n_groups)
+    int32_t skip_dense;         // launch_gather: do not enqueue the dense schedule (the unit's first launch did)
     int32_t ld_cached;          // dense schedule: pixel loads allocate in L1 (1) or not (0)
     int32_t prefetch;           // dense schedule: planes ahead of the front that are prefetched into L2 (0 = off)
     int32_t n_exp_store;        // exposures the store holds from absolute index 0 (bound of the prefetch)
@@ -88,6 +95,7 @@ cudaError_t launch_tiles(const TileParams &t, int sm_count, cudaStream_t stream)
 
 
 
+constexpr int kSlabGroups = 2;          // exposure groups per launch of the slab form of the walk (dt_gather.cuh)
 constexpr int kProgressStride = 32;     // one 128-B line per exposure counter (no false sharing of polls)
 #ifndef DT_K3_THREADS
 #define DT_K3_THREADS 1024

@@ -83,7 +83,7 @@ __device__ __forceinline__ void load_pixel_any(const GatherParams &p, int64_t j,
 template <bool PLANE_VAR, bool EXT>
 __global__ void __launch_bounds__(kSparseThreads) k_gather_sparse(const GatherParams p)
 {
-    if (gather_regime(p) != 0) return;
+    if (gather_regime(p) != p.walk_form) return;
     const int lane = threadIdx.x & 31;
     const int64_t orbit = (int64_t)blockIdx.x * kSparseThreads + threadIdx.x;
     if (orbit >= p.n_pad) return;   // n_pad is a multiple of 32: whole warps leave together
@@ -267,7 +267,7 @@ cudaError_t launch_gather(const GatherParams &p_in, int device, cudaStream_t str
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
-    if (p.lockstep_mode != 0) return launch_gather_dense(p, device, stream);
+    if (p.lockstep_mode != 0 && !p.skip_dense) return launch_gather_dense(p, device, stream);
     return cudaSuccess;
 }
 

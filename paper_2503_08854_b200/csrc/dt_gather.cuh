@@ -70,12 +70,22 @@ __device__ __forceinline__ double div_by_reciprocal(double f, double v, double w
 // Regime of a unit's hit list, decided on the device from kernel 1's hit counter (grid-uniform):
 //   1 dense    at least one hit per 16 pixels of every plane the unit covers: most 128-B lines of a plane are
 //              touched, so the one-exposure-at-a-time lock-step that keeps the plane L2-resident pays;
-//   0 sparse   everything else (every list the five configs produce): the orbit-major walk.
+//   2 slabs    a long list (>= kSlabMinHits per unit; tno+focused: 6.7e7 hits on 1.85e7 lines): the orbit-major
+//              walk, launched once per slab of two exposure groups -- the kernel boundaries keep all warps within 64
+//              exposures of each other, so a line is fetched from DRAM once for most of its hits instead of once
+//              per hit (measured 1.02 -> 0.65 ms per unit); the launches cost ~6 us each, which a short list
+//              (small_mba+focused: 0.15 ms per unit) cannot pay;
+//   0 sparse   everything else: the orbit-major walk in one launch.
+constexpr unsigned long long kSlabMinHits = 25000000ull;
 __device__ __forceinline__ int gather_regime(const GatherParams &p)
 {
-    if (p.lockstep_mode >= 0) return p.lockstep_mode;
+    if (p.lockstep_mode == 1) return 1;
+    if (p.lockstep_mode == 0 && p.slab_mode >= 0) return p.slab_mode;
     const unsigned long long n_hits = p.n_hits_dev ? *p.n_hits_dev : (unsigned long long)p.n_hits_host;
-    return (n_hits * 16ull >= (unsigned long long)p.n_groups * kGroup * (unsigned long long)p.plane) ? 1 : 0;
+    const int ug = p.unit_groups > 0 ? p.unit_groups : p.n_groups;
+    if (p.lockstep_mode < 0 && n_hits * 16ull >= (unsigned long long)ug * kGroup * (unsigned long long)p.plane) return 1;
+    if (p.slab_mode >= 0) return p.slab_mode;
+    return n_hits >= kSlabMinHits ? 2 : 0;
 }
 __device__ __forceinline__ bool gather_is_dense(const GatherParams &p) { return gather_regime(p) == 1; }
 

@@ -349,7 +349,7 @@ def test_more_than_one_orbit_unit():
 
 
 @pytest.mark.parametrize("var_mode", [0, 1], ids=["scalar_var", "plane_var"])
-@pytest.mark.parametrize("schedule", ["auto", "orbit_major", "dense"])
+@pytest.mark.parametrize("schedule", ["auto", "orbit_major", "orbit_major_slabs", "auto_slabs", "dense"])
 def test_gather_hits_entry_matches_definition(schedule, var_mode):
     """dt_gather_hits on a hand-built hit list: every pair hits a seeded random pixel.  Every schedule of
     kernel 3 (forced through dt_set_option) and the library's own choice must give exactly the sequential sums of the definition,
@@ -389,7 +389,10 @@ def test_gather_hits_entry_matches_definition(schedule, var_mode):
     with dt.Tracker(t, ds.observer_ecliptic(t), np.zeros(N), np.zeros(N), W, H, ds.PIXEL_SCALE,
                     variance_mode=var_mode, var_scalar=var_s) as trk:
         trk.load_image_batch(0, flux, var)
-        trk.set_option("gather_schedule", {"auto": -1, "orbit_major": 0, "dense": 1}[schedule])
+        trk.set_option("gather_schedule", {"auto": -1, "orbit_major": 0, "orbit_major_slabs": 0, "auto_slabs": -1,
+                                           "dense": 1}[schedule])
+        if schedule.endswith("_slabs"):          # the walk launched once per exposure group, sums carried between them
+            trk.set_option("gather_slab", 1)
         dS = torch.zeros(n, dtype=torch.float64, device="cuda")
         dW = torch.zeros(n, dtype=torch.float64, device="cuda")
         dc = torch.zeros(n, dtype=torch.int32, device="cuda")
