@@ -498,11 +498,14 @@ def gather_bench(dt, trk, cfg, dev, hbm_gbs, flush, reps=5, regimes=None):
 
 
 # ---- rooflines -------------------------------------------------------------------------------------------------
-def k1_roofline(name, flags, stats, ms_prop, pairs, peak_tf, counts):
-    """Kernel 1 (propagate + project + cull + compact): plain FP64 ALUs.  `achieved` counts every FP64-PIPE
-    instruction the kernel issues (FMA, add, mul, compare, convert alike) as one issue slot = 2 flop, i.e. it is the
-    FP64-pipe utilisation expressed in TFLOP/s, against the DFMA rate measured in this run.  The per-pair count is
-    ncu's for THIS workload and binary (paper_2503_08854_b200/k1_counts.py); without a valid count frac is null."""
+def k1_roofline(name, flags, stats, ms_prop, pairs, peak_tf, counts, issue_peak=None):
+    """Kernel 1 (propagate + project + cull + compact): plain ALUs, two ceilings.  (1) The FP64 pipe: `achieved` counts
+    every FP64-PIPE instruction the kernel issues (FMA, add, mul, compare, convert alike) as one issue slot = 2 flop,
+    i.e. it is the FP64-pipe utilisation expressed in TFLOP/s, against the DFMA rate measured in this run -- what
+    bounds the pairs that are refined.  (2) The issue slots: every warp instruction of whatever pipe against
+    4 schedulers x 1 instruction per clock x SMs x the SM clock -- what bounds the pairs the FP32 group gate removes.
+    `frac` is the FP64 fraction; `issue` holds the second; `binding` names the larger.  The per-pair counts are ncu's
+    for THIS workload and binary (paper_2503_08854_b200/k1_counts.py); without a valid count frac is null."""
     launches = max(stats["propagate_launches"], 1)
     key = name + ("" if flags == 0 else "@flags=%d" % flags)
     rec = counts["workloads"].get(key) if counts["valid"] else None
@@ -519,6 +522,12 @@ def k1_roofline(name, flags, stats, ms_prop, pairs, peak_tf, counts):
     r.update(achieved=achieved, frac=achieved / peak_tf if peak_tf else None, fp64_slots_per_pair=slots,
              inst_per_pair=rec["inst_per_pair"],
              note="FP64-pipe utilisation: ncu smsp__inst_executed_pipe_fp64 per pair of this workload x pairs / time")
+    if issue_peak:
+        rate = rec["inst_per_pair"] / 32.0 * pairs / (ms_prop * 1e-3)             # warp instructions per second
+        r["issue"] = {"achieved": rate * 1e-9, "peak": issue_peak * 1e-9, "unit": "G warp-instructions/s",
+                      "frac": rate / issue_peak,
+                      "peak_source": "SMs x 4 schedulers x 1 instruction per clock x max SM clock (B200_PROFILING.md)"}
+        r["binding"] = "issue" if r["issue"]["frac"] > (r["frac"] or 0.0) else "fp64"
     return r
 
 
@@ -532,6 +541,8 @@ def combined_roofline(w, stats, ms_step, ms_prop, u, k1, hbm_gbs, h2d_gbs, peak_
     bytes_min = n * 48 + n * 12 + pairs / 8 + hits * 8 + hits * sect_per_hit * 32 + touched * 20
     t_hbm = bytes_min / (hbm_gbs * 1e9)
     t_fp64 = (k1["fp64_slots_per_pair"] * pairs / (peak_tf * 1e12 / 2.0)) if k1.get("fp64_slots_per_pair") else None
+    if t_fp64 is not None and k1.get("issue"):            # the ALU roof of kernel 1 is the slower of its two ceilings
+        t_fp64 = max(t_fp64, k1["inst_per_pair"] / 32.0 * pairs / (k1["issue"]["peak"] * 1e9))
     t_h2d = stats["h2d_image_bytes"] / (h2d_gbs * 1e9) if h2d_gbs else 0.0
     roof = (max(t_fp64, t_hbm) if t_fp64 is not None else None)
     out = {"bytes_min": bytes_min, "t_hbm_ms": t_hbm * 1e3, "t_fp64_ms": None if t_fp64 is None else t_fp64 * 1e3,
@@ -598,7 +609,9 @@ def run_config(dt, args, name, dev, local_rank, rank, world, steps, warmup, flus
             entry["clocks"] = clocks
         u = None
         if rank == 0:
-            k1 = k1_roofline(cfg.name, args.flags, stats, ms_prop, pairs_rank, peaks["fp64_tf"], counts)
+            import torch
+            issue_peak = torch.cuda.get_device_properties(dev).multi_processor_count * 4 * sm_clock_hz(local_rank)
+            k1 = k1_roofline(cfg.name, args.flags, stats, ms_prop, pairs_rank, peaks["fp64_tf"], counts, issue_peak)
             entry["fp64_tflops"] = k1["achieved"]
             entry["k1_roofline"] = k1
             if with_gather and stats["hits"] > 0 and not w.beyond_hbm:
