@@ -83,6 +83,7 @@ struct dt_context {
     int64_t mask_cap = 0, base_cap = 0, off_cap = 0;
     unsigned long long *d_counters = nullptr;           // [8]
     GatePolicy *d_policy = nullptr;                     // kernel-1 variant of the next unit (device-side choice)
+    unsigned long long *h_max_hits = nullptr, *d_max_hits = nullptr;   // largest unit hit count seen: mapped host word
     int32_t group_gate = -1;                            // -1 chosen on the device, 0 never, 1 always
     int32_t gather_slab = -1;                           // walk in slabs: -1 chosen on the device, 0 never, k: always, k groups
     int *d_progress = nullptr;                          // kernel 3 lock-step counters, one per exposure of a unit
@@ -186,6 +187,7 @@ void free_all(dt_context *c)
     cudaFree(c->d_els); cudaFree(c->d_t0s); cudaFree(c->d_Ss); cudaFree(c->d_Wts); cudaFree(c->d_cnts);
     cudaFree(c->d_perm); cudaFree(c->d_skey); cudaFree(c->d_sort_tmp);
     cudaFree(c->d_policy);
+    if (c->h_max_hits) cudaFreeHost(c->h_max_hits);
     cudaFree(c->d_progress);
     cudaFree(c->tile_count);
     cudaFree(c->tile_slot);
@@ -384,6 +386,11 @@ int dt_create(const dt_survey *s, dt_context **out)
                             c->stream) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
         if (cudaMalloc((void **)&c->d_counters, 8 * sizeof(unsigned long long)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
         if (cudaMalloc((void **)&c->d_policy, sizeof(GatePolicy)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
+        if (cudaHostAlloc((void **)&c->h_max_hits, sizeof(unsigned long long), cudaHostAllocMapped) == cudaSuccess) {
+            *c->h_max_hits = 0;
+            if (cudaHostGetDevicePointer((void **)&c->d_max_hits, c->h_max_hits, 0) != cudaSuccess) c->d_max_hits = nullptr;
+        }
+        cudaGetLastError();                                       // without the word: no hint, every form is enqueued
         {
             const GatePolicy first = {1, 0, 0ull, 0ull};          // a context starts with the gate on
             if (cudaMemcpy(c->d_policy, &first, sizeof first, cudaMemcpyHostToDevice) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
@@ -507,15 +514,19 @@ static cudaError_t launch_k1_unit(dt_context *c, PropagateParams &p, int mode, i
     const bool can_gate = mode == (kModeWarm | kModePrecull);
     const int gate = (!can_gate || (c->flags & DT_FLAG_NO_GROUP_GATE)) ? 0 : c->group_gate;
     p.policy = nullptr;
+    cudaError_t e;
     if (gate >= 0) {
-        *launches += 1;
-        return launch_propagate(p, gate ? (mode | kModeGate) : mode, c->stream);
+        *launches += 2;
+        e = launch_propagate(p, gate ? (mode | kModeGate) : mode, c->stream);
+    } else {
+        p.policy = c->d_policy;
+        e = launch_propagate(p, mode | kModeGate, c->stream);
+        if (e == cudaSuccess) e = launch_propagate(p, mode, c->stream);
+        *launches += 3;
     }
-    p.policy = c->d_policy;
-    cudaError_t e = launch_propagate(p, mode | kModeGate, c->stream);
-    if (e == cudaSuccess) e = launch_propagate(p, mode, c->stream);
-    if (e == cudaSuccess) e = launch_gate_policy(c->d_policy, c->d_counters, p.n_orbits * (int64_t)p.n_exp, c->stream);
-    *launches += 3;
+    // one thread: the next unit's variant, and the largest unit hit count seen (the host's hint for kernel 3)
+    if (e == cudaSuccess)
+        e = launch_gate_policy(c->d_policy, c->d_counters, p.n_orbits * (int64_t)p.n_exp, c->d_max_hits, c->stream);
     return e;
 }
 
@@ -530,6 +541,13 @@ static cudaError_t launch_gather_unit(const dt_context *c, const GatherParams &g
     if (g.flux_ptrs || ext) g.lockstep_mode = 0;                       // as launch_gather: walk only
     int32_t slab_opt = c->gather_slab;                                 // -1 auto, 0 never, k > 0: always, k groups
     if (g.flux_ptrs || g.lockstep_mode == 1) slab_opt = 0;             // pixels over PCIe / dense forced: no slabs
+    // the slab launches cost a few microseconds each even when they return at once: they are enqueued only once the
+    // context has produced a unit with 80 % of the hits the slab regime takes (a hint read without synchronising:
+    // a stale or missing value only changes which of two equivalent forms runs)
+    if (slab_opt < 0 && c->h_max_hits && g.n_hits_dev &&
+        *(volatile unsigned long long *)c->h_max_hits < kSlabMinHits / 5 * 4)
+        slab_opt = 0;
+    if (slab_opt < 0 && !g.n_hits_dev && (unsigned long long)g.n_hits_host < kSlabMinHits) slab_opt = 0;   // known here
     const int32_t slab = slab_opt > 0 ? slab_opt : kSlabGroups;
     if (slab_opt == 0 || slab >= g.n_groups) {
         g.slab_mode = 0;

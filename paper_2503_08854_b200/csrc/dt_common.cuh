@@ -95,6 +95,7 @@ cudaError_t launch_tiles(const TileParams &t, int sm_count, cudaStream_t stream)
 
 
 
+constexpr unsigned long long kSlabMinHits = 25000000ull;   // hits per unit from which the slab form pays
 constexpr int kSlabGroups = 2;          // exposure groups per launch of the slab form of the walk (dt_gather.cuh)
 constexpr int kProgressStride = 32;     // one 128-B line per exposure counter (no false sharing of polls)
 #ifndef DT_K3_THREADS

@@ -76,7 +76,6 @@ __device__ __forceinline__ double div_by_reciprocal(double f, double v, double w
 //              per hit (measured 1.02 -> 0.65 ms per unit); the launches cost ~6 us each, which a short list
 //              (small_mba+focused: 0.15 ms per unit) cannot pay;
 //   0 sparse   everything else: the orbit-major walk in one launch.
-constexpr unsigned long long kSlabMinHits = 25000000ull;
 __device__ __forceinline__ int gather_regime(const GatherParams &p)
 {
     if (p.lockstep_mode == 1) return 1;

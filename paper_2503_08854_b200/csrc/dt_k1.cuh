@@ -80,8 +80,11 @@ struct GatePolicy {
     int32_t cooldown;               // units left before a gate that proved useless is tried again
     unsigned long long refined0, gated0;   // counters[1], counters[6] at the end of the previous unit
 };
+// max_unit_hits: NULL, or a word in device-mapped page-locked HOST memory that holds the largest hit count of any unit
+// the context has processed: a hint the host reads, without synchronising, to decide which forms of kernel 3 are
+// worth enqueueing at all (dt_api.cu launch_gather_unit); never a result.
 cudaError_t launch_gate_policy(GatePolicy *policy, const unsigned long long *counters, int64_t unit_pairs,
-                               cudaStream_t stream);
+                               unsigned long long *max_unit_hits, cudaStream_t stream);
 
 cudaError_t launch_propagate(const PropagateParams &p, int mode, cudaStream_t stream);
 

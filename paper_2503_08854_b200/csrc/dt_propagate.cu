@@ -538,8 +538,13 @@ cudaError_t launch_propagate(const PropagateParams &p, int mode, cudaStream_t st
 // The gate pays where the warps cull (a blind search) and its remainder bounds are tight enough to gate; it costs
 // where most pairs are refined anyway (a focused search: the variant without it is the faster binary there) or where
 // the bounds are loose (eccentric near-Earth orbits).  Both are read off what the unit just did.
-__global__ void k_gate_policy(GatePolicy *pol, const unsigned long long *counters, long long unit_pairs)
+__global__ void k_gate_policy(GatePolicy *pol, const unsigned long long *counters, long long unit_pairs,
+                              unsigned long long *max_unit_hits)
 {
+    if (max_unit_hits && counters[0] > *max_unit_hits) {
+        *max_unit_hits = counters[0];
+        __threadfence_system();
+    }
     const unsigned long long refined = counters[1] - pol->refined0, gated = counters[6] - pol->gated0;
     pol->refined0 = counters[1];
     pol->gated0 = counters[6];
@@ -554,9 +559,9 @@ __global__ void k_gate_policy(GatePolicy *pol, const unsigned long long *counter
 }
 
 cudaError_t launch_gate_policy(GatePolicy *policy, const unsigned long long *counters, int64_t unit_pairs,
-                               cudaStream_t stream)
+                               unsigned long long *max_unit_hits, cudaStream_t stream)
 {
-    k_gate_policy<<<1, 1, 0, stream>>>(policy, counters, (long long)unit_pairs);
+    k_gate_policy<<<1, 1, 0, stream>>>(policy, counters, (long long)unit_pairs, max_unit_hits);
     return cudaGetLastError();
 }
 
