@@ -195,7 +195,11 @@ __global__ void __launch_bounds__(kSparseThreads) k_gather_sparse(const GatherPa
                             if (PLANE_VAR) vv[q] = ld_pixel_cached(p.var_ptrs[j0 + jj[q]] + off[q]);
                         }
                     } else if (PLANE_VAR && p.fv) {
-                        const float2 t2 = ld_pixel2_64(p.fv + ((j0 + jj[q]) * p.plane + off[q]));
+                        // a miss fetches 64 B of DRAM in the one-launch walk (no other hit of the line will find it in
+                        // the L2: half the bytes at the same access rate) and the whole 128-B line in the slab form, where
+                        // the line's other hits come by while it is resident: fewer DRAM accesses, which is what bounds
+                        const float2 *a2 = p.fv + ((j0 + jj[q]) * p.plane + off[q]);
+                        const float2 t2 = (p.walk_form == 2) ? ld_pixel2_cached(a2) : ld_pixel2_64(a2);
                         f[q] = t2.x;
                         vv[q] = t2.y;
                     } else {
