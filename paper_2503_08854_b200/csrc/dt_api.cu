@@ -84,6 +84,7 @@ struct dt_context {
     unsigned long long *d_counters = nullptr;           // [8]
     GatePolicy *d_policy = nullptr;                     // kernel-1 variant of the next unit (device-side choice)
     unsigned long long *h_max_hits = nullptr, *d_max_hits = nullptr;   // largest unit hit count seen: mapped host word
+    float4 *d_group_bounds = nullptr;                   // [3 x exposure groups]: the gate's group-level bounds of a launch
     int32_t group_gate = -1;                            // -1 chosen on the device, 0 never, 1 always
     int32_t gather_slab = -1;                           // walk in slabs: -1 chosen on the device, 0 never, k: always, k groups
     int *d_progress = nullptr;                          // kernel 3 lock-step counters, one per exposure of a unit
@@ -187,6 +188,7 @@ void free_all(dt_context *c)
     cudaFree(c->d_els); cudaFree(c->d_t0s); cudaFree(c->d_Ss); cudaFree(c->d_Wts); cudaFree(c->d_cnts);
     cudaFree(c->d_perm); cudaFree(c->d_skey); cudaFree(c->d_sort_tmp);
     cudaFree(c->d_policy);
+    cudaFree(c->d_group_bounds);
     if (c->h_max_hits) cudaFreeHost(c->h_max_hits);
     cudaFree(c->d_progress);
     cudaFree(c->tile_count);
@@ -386,6 +388,7 @@ int dt_create(const dt_survey *s, dt_context **out)
                             c->stream) != cudaSuccess) { rc = DT_ERR_CUDA; break; }
         if (cudaMalloc((void **)&c->d_counters, 8 * sizeof(unsigned long long)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
         if (cudaMalloc((void **)&c->d_policy, sizeof(GatePolicy)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
+        if (cudaMalloc((void **)&c->d_group_bounds, sizeof(float4) * 3 * (size_t)((s->n_exposures + kGroup - 1) / kGroup + 1)) != cudaSuccess) { rc = DT_ERR_OOM; break; }
         if (cudaHostAlloc((void **)&c->h_max_hits, sizeof(unsigned long long), cudaHostAllocMapped) == cudaSuccess) {
             *c->h_max_hits = 0;
             if (cudaHostGetDevicePointer((void **)&c->d_max_hits, c->h_max_hits, 0) != cudaSuccess) c->d_max_hits = nullptr;
@@ -604,6 +607,7 @@ static void fill_common(const dt_context *c, PropagateParams &p, double t0)
     p.width = c->W;
     p.tan_fov = c->tan_fov;
     p.offsets_cap = c->off_cap;
+    p.group_bounds = c->d_group_bounds;
 }
 
 static int32_t pick_groups_per_split(int64_t n_orbits, int32_t n_exp)

@@ -65,6 +65,8 @@ struct PropagateParams {
     int64_t offsets_cap;        // entries `offsets` can hold (bounds-check build)
     unsigned long long *counters;  // [0] unit hit allocator, [1] refined pairs, [2] cold solves, [3] hits, [4] sub-step solves, [6] gated pairs, [7] bounds violations
     const GatePolicy *policy;   // NULL, or: the kernel returns at once unless policy->select says its variant runs
+    float4 *group_bounds;       // NULL, or device [3 x exposure groups of the launch]: written by launch_propagate
+                                // (k_group_bounds) for the gate variant's group-level test (dt_orbit.cuh group_is_far)
     // dense debug outputs (dt_project), NULL on the timed path
     double *radec, *xy;         // [n][n_exp][2]
     int32_t *pix;               // [n][n_exp][2]

@@ -588,4 +588,30 @@ __device__ __forceinline__ bool group_gate_culls(const GroupEph &G, float tau, f
     return (D0 < -G.eps) || (fmaf(-D0, D0, r2) > fmaf(w, w, 40.0f * kGateU * r2));
 }
 
+// ---- group-level test: can the orbit be near ANY exposure of the group? ---------------------------------------------
+// Where a group's pointings cluster (a survey that follows the opposition point), most orbits are nowhere near any of its
+// 32 exposures, and one test per (orbit, group) replaces 32.  Per group (k_group_bounds, once per launch): the axis c of the
+// pointings, alpha = 1.01 theta_c + max_j angle(t_j, c) + 1e-4, the mean observer position R_m and dR = max_j |R_j - R_m|.
+// The retarded topocentric vector of exposure j is p_j = [r(t_m) - R_m] + [r(t_j - lt) - r(t_m)] - [R_j - R_m], i.e. within
+// rho_b = v_max (tau_max + lt) + dR of p_m = r(t_m) - R_m (speed bound; lt <= (|p_m| + rho_b) / c), so its direction is within
+// asin(rho_b / |p_m|) of p_m's, and a hit needs angle(p_j, t_j) <= theta_c.  Hence no exposure of the group can be hit when
+//     angle(p_m, c) > alpha + asin(rho_b / |p_m|) =: Theta   (Theta < pi / 2),
+// tested as p_m . c < |p_m| cos(Theta) with cos(Theta) = cos(alpha) sqrt(1 - s^2) - sin(alpha) s, s = rho_b / |p_m| < 1.
+// FP32 with margins: 1e-4 AU on rho_b for the rounding of p_m (<= 1e-5 AU at 50 AU), 1e-5 relative and 1e-6 AU absolute on
+// the comparison.  bounds: (c, cos alpha), (R_m, dR), (sin alpha, -, -, -); cos alpha = -2 marks a group without a usable cone.
+__device__ __forceinline__ bool group_is_far(float rx, float ry, float rz, float vmax, float tau_max, float inv_c,
+                                             float4 b0, float4 b1, float4 b2)
+{
+    const float px = rx - b1.x, py = ry - b1.y, pz = rz - b1.z;
+    const float pm2 = fmaf(px, px, fmaf(py, py, pz * pz));
+    const float pm = sqrtf(pm2);
+    float rho_b = fmaf(vmax, tau_max, b1.w) + 1e-4f;
+    rho_b = fmaf(1.05f * vmax * inv_c, pm + 2.f * rho_b, rho_b);        // light-time: v_max (|p_m| + rho_b) / c, with room
+    const float s = rho_b / pm;
+    const float cosT = fmaf(b0.w, sqrtf(fmaxf(1.f - s * s, 0.f)), -b2.x * s);
+    const float pc = fmaf(px, b0.x, fmaf(py, b0.y, pz * b0.z));
+    // written so that a NaN anywhere means "not far"
+    return (s < 0.98f) && (b0.w > -1.f) && (cosT > 1e-3f) && (pc < fmaf(pm, cosT * (1.f - 1e-5f), -1e-6f));
+}
+
 }  // namespace dt

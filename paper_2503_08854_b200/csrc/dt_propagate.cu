@@ -133,6 +133,7 @@ __global__ void __launch_bounds__(kTileOrbits, (MODE & kModeGate) ? DT_K1_GATE_C
         }
 
         bool gate_ready = false, gate_off = false;   // warp-uniform: this group's ephemeris exists / is of no use
+        bool group_far = false;                      // warp-uniform: no lane can be near ANY exposure of the group
         uint32_t bits = 0;
         int cnt = 0;          // this lane's hits in the group
         int run = 0;          // the warp's hits in the group so far (warp-uniform)
@@ -217,7 +218,28 @@ __global__ void __launch_bounds__(kTileOrbits, (MODE & kModeGate) ? DT_K1_GATE_C
                         sm.geph[10][tid] = G.eps;
                         gate_off = !__all_sync(0xffffffffu, G.eps < (float)kGateEpsMax);
                         __syncwarp();
+                        // one test for the whole group, where its pointings cluster (dt_orbit.cuh group_is_far)
+                        if (p.group_bounds) {
+                            const float4 b0 = p.group_bounds[3 * g], b1 = p.group_bounds[3 * g + 1],
+                                         b2 = p.group_bounds[3 * g + 2];
+                            group_far = __all_sync(0xffffffffu,
+                                                   !o.valid || group_is_far(G.rx, G.ry, G.rz, __double2float_ru(o.vmax),
+                                                                            __double2float_ru(tau_max),
+                                                                            __double2float_ru(p.inv_c), b0, b1, b2));
+                        }
                     }
+                }
+                if (group_far) {
+                    if (DENSE && in_range) {              // dt_project: gated pairs are reported as culled
+                        for (int q = jj; q < nrec; ++q) {
+                            const int64_t k = (orbit * p.n_exp + (int64_t)g * kGroup + q) * 2;
+                            if (p.radec) p.radec[k] = p.radec[k + 1] = nan("");
+                            if (p.xy) p.xy[k] = p.xy[k + 1] = nan("");
+                            if (p.pix) p.pix[k] = p.pix[k + 1] = -1;
+                        }
+                    }
+                    n_gated += (unsigned)(nrec - jj);
+                    break;
                 }
                 if (!gate_off) {
                     GroupEph G;
@@ -505,6 +527,8 @@ __global__ void __launch_bounds__(kTileOrbits, (MODE & kModeGate) ? DT_K1_GATE_C
     }
 }
 
+__global__ void k_group_bounds(const ExpRec *exp, int n_exp, double tan_fov, float4 *out);
+
 template <int MODE>
 static cudaError_t launch_mode(const PropagateParams &p, cudaStream_t stream)
 {
@@ -512,6 +536,8 @@ static cudaError_t launch_mode(const PropagateParams &p, cudaStream_t stream)
     const int n_groups = (p.n_exp + kGroup - 1) / kGroup;
     const int splits = (n_groups + p.groups_per_split - 1) / p.groups_per_split;
     dim3 grid((unsigned)((p.n_orbits + kTileOrbits - 1) / kTileOrbits), (unsigned)splits);
+    if ((MODE & kModeGate) && p.group_bounds)
+        k_group_bounds<<<(unsigned)n_groups, 32, 0, stream>>>(p.exp, p.n_exp, p.tan_fov, p.group_bounds);
     k_propagate<MODE><<<grid, kTileOrbits, smem, stream>>>(p);
     return cudaGetLastError();
 }
@@ -531,6 +557,45 @@ cudaError_t launch_propagate(const PropagateParams &p, int mode, cudaStream_t st
         case 11: return launch_mode<11>(p, stream);
         case 15: return launch_mode<15>(p, stream);
         default: return cudaErrorInvalidValue;
+    }
+}
+
+// ---- per-group bounds of the gate's group-level test (dt_orbit.cuh group_is_far): one warp per exposure group ----
+__global__ void __launch_bounds__(32) k_group_bounds(const ExpRec *exp, int n_exp, double tan_fov, float4 *out)
+{
+    const int g = blockIdx.x, lane = threadIdx.x;
+    const int nrec = min(kGroup, n_exp - g * kGroup);
+    const bool have = lane < nrec;
+    const ExpRec x = exp[g * kGroup + min(lane, nrec - 1)];
+    double sx = have ? x.tx : 0.0, sy = have ? x.ty : 0.0, sz = have ? x.tz : 0.0;
+    double mx = have ? x.Rx : 0.0, my = have ? x.Ry : 0.0, mz = have ? x.Rz : 0.0;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        sx += __shfl_xor_sync(0xffffffffu, sx, d);
+        sy += __shfl_xor_sync(0xffffffffu, sy, d);
+        sz += __shfl_xor_sync(0xffffffffu, sz, d);
+        mx += __shfl_xor_sync(0xffffffffu, mx, d);
+        my += __shfl_xor_sync(0xffffffffu, my, d);
+        mz += __shfl_xor_sync(0xffffffffu, mz, d);
+    }
+    const double sn = sqrt(fma(sx, sx, fma(sy, sy, sz * sz)));
+    const bool axis = sn > 1e-3 * nrec;                       // pointings all around the sky: no axis
+    const double cx = axis ? sx / sn : 1.0, cy = axis ? sy / sn : 0.0, cz = axis ? sz / sn : 0.0;
+    mx /= nrec; my /= nrec; mz /= nrec;
+    double cmin = have ? fma(x.tx, cx, fma(x.ty, cy, x.tz * cz)) : 1.0;                       // cos angle(t_j, c)
+    const double ex = x.Rx - mx, ey = x.Ry - my, ez = x.Rz - mz;
+    double dmax = have ? sqrt(fma(ex, ex, fma(ey, ey, ez * ez))) : 0.0;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        cmin = fmin(cmin, __shfl_xor_sync(0xffffffffu, cmin, d));
+        dmax = fmax(dmax, __shfl_xor_sync(0xffffffffu, dmax, d));
+    }
+    if (lane == 0) {
+        const double alpha = 1.01 * atan(tan_fov) + acos(fmin(fmax(cmin, -1.0), 1.0)) * 1.0001 + 1e-4;
+        const bool ok = axis && alpha < 1.5 && isfinite(alpha) && isfinite(dmax);
+        out[3 * g] = make_float4((float)cx, (float)cy, (float)cz, ok ? __double2float_rd(cos(alpha)) : -2.f);
+        out[3 * g + 1] = make_float4((float)mx, (float)my, (float)mz, __double2float_ru(dmax * 1.0001 + 1e-6));
+        out[3 * g + 2] = make_float4(ok ? __double2float_ru(sin(alpha)) : 1.f, 0.f, 0.f, 0.f);
     }
 }
 
