@@ -811,3 +811,51 @@ def test_sky_order_changes_nothing_but_rounding(case):
     a, b = res[0][0][same], res[1][0][same]
     ok = (np.isnan(a) & np.isnan(b)) | (np.abs(a - b) <= 1e-9 * np.maximum(np.abs(b), 1e-3))
     assert ok.all()
+
+
+def test_group_level_gate_against_oracle():
+    """The group-level test of the gate (one bounding-cone test per orbit and group where a group's pointings cluster:
+    dt_orbit.cuh group_is_far) on the survey geometry that switches it on -- pointings that follow the opposition
+    point, configs[1] at full cadence -- with pixels 100 times coarser than the configs', so that a blind set of
+    main-belt orbits has over a thousand oracle hits to lose: none may be removed, survivors keep full precision, and the
+    test must really remove most (orbit, group) pairs."""
+    dt = _dt()
+    cfg = ds.scaled(ds.CONFIGS["small_mba"], n_orbits=8192, width=512, height=384)
+    sc = ds.build_scene(cfg, oracle.scene_project_fn, inject=False)
+    scale = 100.0 * sc.pixel_scale                         # 20 arcsec per pixel: a 2.8 x 2.1 degree footprint
+    el = sc.elements()
+    srv = oracle.Survey(sc.t, sc.obs_ecl, sc.ra0, sc.dec0, cfg.width, cfg.height, scale, sc.gm, sc.c, sc.obliquity)
+    ref = oracle.project(srv, el, sc.t0)
+    ohit = ref["pix"][..., 0] >= 0
+    assert int(ohit.sum()) > 1000, int(ohit.sum())
+    fr = {}
+    for flags in (8, 24):
+        with dt.Tracker(sc.t, sc.obs_ecl, sc.ra0, sc.dec0, cfg.width, cfg.height, scale, gm=sc.gm, c=sc.c,
+                        obliquity=sc.obliquity, variance_mode=0, var_scalar=np.ones(cfg.n_exp), flags=flags) as trk:
+            out = trk.project(el, sc.t0)
+        refined = np.isfinite(out["radec"][..., 0])
+        assert not (ohit & ~refined).any(), (flags, np.argwhere(ohit & ~refined)[:5])
+        assert (out["pix"][~refined] == -1).all()
+        sub = dict(radec=np.where(refined[..., None], out["radec"], ref["radec"]),
+                   xy=np.where(refined[..., None], out["xy"], ref["xy"]),
+                   pix=np.where(refined[..., None], out["pix"], ref["pix"]))
+        _compare_project(sub, ref)
+        fr[flags] = float(refined.mean())
+    assert fr[8] <= fr[24] + 1e-12
+    # dt_stack statistics on the same geometry: most pairs gated, same hits with and without
+    flux = np.zeros((cfg.n_exp, cfg.height, cfg.width), np.float32)
+    st = {}
+    for gate in (1, 0):
+        with dt.Tracker(sc.t, sc.obs_ecl, sc.ra0, sc.dec0, cfg.width, cfg.height, scale, gm=sc.gm, c=sc.c,
+                        obliquity=sc.obliquity, variance_mode=0, var_scalar=np.ones(cfg.n_exp)) as trk:
+            trk.set_option("group_gate", gate)
+            trk.load_image_batch(0, flux, None)
+            snr, hits = trk.stack(el, sc.t0)
+            st[gate] = (np.array(hits), trk.stats())
+    assert np.array_equal(st[1][0], st[0][0])
+    clean = ref["flag"].sum(-1) == 0
+    assert np.array_equal(st[1][0][clean], ohit.sum(-1)[clean])
+    assert st[1][1]["gated_pairs"] > 0.6 * st[1][1]["pairs"], st[1][1]
+    parity_record("group_level_gate", pairs=int(ohit.size), oracle_hits=int(ohit.sum()),
+                  refined_fraction_gate=fr[8], refined_fraction_no_gate=fr[24],
+                  gated_fraction=st[1][1]["gated_pairs"] / st[1][1]["pairs"])
