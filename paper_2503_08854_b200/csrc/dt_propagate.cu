@@ -27,7 +27,8 @@ namespace dt {
 #define DT_K1_GATE_CTAS 5          // the gate variant: its hot loop is latency-bound, one more CTA per SM pays
 #endif
 constexpr int kMaxSubsteps = 6;    // wide sub-steps of one Kepler step before the cold solve is cheaper
-constexpr double kGateEpsMax = 0.03;   // AU: a looser remainder bound in the warp switches the group's gate off
+constexpr double kGateEpsMax = 0.35;   // AU: a looser remainder bound in the warp switches the group's gate off (the test
+                                       // still removes every pair farther than ~eps / distance from the pointing)
 
 struct __align__(128) PropSmem {
     ExpRec rec[2][kGroup];                       // 8 KB: two-slot ring of exposure groups

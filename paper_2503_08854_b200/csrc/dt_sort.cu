@@ -25,7 +25,11 @@ namespace {
 
 constexpr int kSortThreads = 256;
 constexpr int kBandBits = 9, kRaBits = 11;          // 512 x 2048 equal-area cells
-constexpr int kKeyBits = kBandBits + kRaBits;
+constexpr int kKeyBits = kBandBits + kRaBits + 1;    // + 1: orbits with a perihelion inside kLoosePerihelion sort last
+// The group ephemeris gate of kernel 1 decides per warp and needs every lane's remainder bound to be tight; the bound grows
+// like 1 / r^3, so ONE orbit that comes close to the Sun switches the gate off for its 31 neighbours.  Orbits whose
+// perihelion lies inside 0.7 AU are therefore kept apart from the others (only the near-Earth config has any).
+constexpr double kLoosePerihelion = 0.7;
 
 // apparent direction (geometric, no light-time: a sort key, not a result) at the key exposure -> cell index
 __global__ void __launch_bounds__(kSortThreads) k_sky_keys(const double *__restrict__ elements,
@@ -57,6 +61,7 @@ __global__ void __launch_bounds__(kSortThreads) k_sky_keys(const double *__restr
         const uint32_t band = min((uint32_t)((z + 1.0) * 0.5 * (double)(1 << kBandBits)), (1u << kBandBits) - 1u);
         const uint32_t cell = min((uint32_t)(ra * (double)(1 << kRaBits)), (1u << kRaBits) - 1u);
         key = (band << kRaBits) | cell;
+        if (el[0] * (1.0 - el[1]) < kLoosePerihelion) key |= 1u << (kBandBits + kRaBits);
     }
     if (i < n) {
         keys[i] = key;
