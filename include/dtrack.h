@@ -320,7 +320,8 @@ int dt_filter_intersections(dt_context *ctx, const double *elements, int64_t n, 
  * dt_sky_order: the order dt_stack processes one unit of orbits in (option "sort_orbits"; csrc/dt_sort.cu): position i
  * of the sorted unit holds orbit perm_out[i].  elements [n][6] fp64 and t0_orbit [n] (or NULL: the scalar t0) are
  * DEVICE arrays, n <= 2^20 (one unit), perm_out [n] uint32 a DEVICE array.  The key of an orbit is the equal-area
- * sky cell (512 x 2048) of its geometric direction from the observer at the survey's middle exposure; the sort is
+ * sky cell (512 x 2048) of its geometric direction from the observer at the survey's middle exposure (orbits with a
+ * perihelion inside 0.7 AU sort after all others); the sort is
  * stable, so the permutation is a pure function of the input.  A measurement / test entry: the kernel-1 and
  * kernel-3 entries (dt_filter_intersections, dt_gather_hits) work on the order they are given, and a caller that
  * wants what dt_stack runs passes them elements[perm].  Synchronises the context stream.

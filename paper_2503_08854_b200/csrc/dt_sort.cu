@@ -12,7 +12,7 @@
 // nothing outside this file sees the permutation.  Orbits that belong together (the members of a family around a
 // known object, neighbouring nodes of a search grid) end up in the same warps whatever order they came in.
 //
-// The sort itself is library code (CUB's DeviceRadixSort, 20-bit keys, ~0.1 ms per unit against milliseconds of
+// The sort itself is library code (CUB's DeviceRadixSort, 21-bit keys, ~0.1 ms per unit against milliseconds of
 // kernel 1): it orders work, it computes nothing of the method.
 #include <cub/device/device_radix_sort.cuh>
 
