@@ -66,6 +66,7 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-gather-bench", action="store_true")
     ap.add_argument("--gather-only", action="store_true", help="run only the kernel-3 micro-benchmarks")
+    ap.add_argument("--option", action="append", help="dt_set_option name=value on the workload's context (repeatable)")
     ap.add_argument("--gather-slab", type=int, default=-1, help="dt_set_option gather_slab / gather_schedule 0 (experiments)")
     ap.add_argument("--gather-reps", type=int, default=5, help="timed repetitions per kernel-3 regime")
     ap.add_argument("--gather-regimes", default="", help="comma-separated subset of the kernel-3 regimes")
@@ -580,6 +581,9 @@ def run_config(dt, args, name, dev, local_rank, rank, world, steps, warmup, flus
         cfg = ds.focused(cfg)
     t_build = time.perf_counter()
     w = Workload(dt, cfg, dev, local_rank, rank, world, flags=args.flags)
+    for kv in (args.option or []):                    # dt_set_option name=value (tuning experiments)
+        k, _, v = kv.partition("=")
+        w.trk.set_option(k, int(v))
     t_build = time.perf_counter() - t_build
     try:
         sampler = ClockSampler(local_rank) if (sample_clocks and rank == 0) else None     # the timed region only

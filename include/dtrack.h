@@ -347,7 +347,7 @@ int dt_sky_order(dt_context *ctx, const double *elements_dev, const double *t0_o
  *   "gather_l1"           dense schedule: 1 pixel loads allocate in L1, 0 they do not
  *   "stream_tiles"        streaming mode: -1 / 1 use the tiled image cache when the planes are device-mappable
  *                         (default), 0 stream whole planes in double-buffered batches; "tile_min_hits": hits of
- *                         one orbit unit on a tile from which the tile is fetched (0 = tile bytes / 256)
+ *                         one orbit unit on a tile from which the tile is fetched (0 = tile bytes / 1024)
  *   "stream_zero_copy"    streaming mode: -1 probe the hit density (default), 0 always copy batches, 1 always
  *                         gather from the pinned planes
  *   "zero_copy_elements"  1 kernel 1 reads DT_MEM_PINNED elements in place (default), 0 copies them first
